@@ -1,0 +1,481 @@
+"""Pins of the fp64 oracle to things other than itself (CPU only).
+
+Every test names the pin (P1..P14 of SURVEY.md section 8(c) / DESIGN.md) and the
+paper passage that fixes the expected value.  The expected values come from:
+the paper's printed numbers (tests/golden/paper_values.txt), closed forms,
+mpmath extended precision, numpy's own FFT (a different library routine from
+the oracle's radix-2), and brute force on tiny inputs.
+"""
+import math
+import os
+
+import mpmath
+import numpy as np
+import pytest
+
+import datagen
+import oracle
+
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")) as fh:
+    for line in fh:
+        line = line.split("#")[0].strip()
+        if "=" in line:
+            k, v = line.split("=")
+            GOLD[k.strip()] = float(v)
+
+D_HZ = GOLD["D_MHZ2_US"] * 1e12 * 1e-6  # MHz^2 us -> Hz^2 s
+
+
+def cfg_tiny(**kw):
+    base = dict(n_chan=64, bw_hz=16e6, f_center_hz=325e6, dm=(10.0,), n_fft=1024, n_int=16)
+    base.update(kw)
+    return oracle.OracleConfig(**base)
+
+
+# ----------------------------------------------------------------------------- P1: transforms
+@pytest.mark.parametrize("n", [1, 2, 4, 8, 16, 32, 64])
+def test_p1_radix2_equals_bruteforce_dft(n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    for sign in (-1, +1):
+        a = oracle.fft(x, sign, force_radix2=True)
+        b = oracle.dft_naive(x, sign)
+        assert np.max(np.abs(a - b)) < 1e-12 * max(1.0, np.max(np.abs(b)))
+
+
+@pytest.mark.parametrize("n", [3, 5, 12, 64])
+def test_p1_naive_dft_is_the_definition(n):
+    """Naive DFT against the DFT matrix written out with mpmath (definition, sign convention)."""
+    rng = np.random.default_rng(100 + n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    got = oracle.dft_naive(x, -1)
+    mpmath.mp.dps = 30
+    for k in (0, 1, n - 1):
+        acc = mpmath.mpc(0)
+        for m in range(n):
+            acc += mpmath.mpc(x[m]) * mpmath.e ** (-2j * mpmath.pi * k * m / n)
+        assert abs(complex(acc) - got[k]) < 1e-12
+
+
+@pytest.mark.parametrize("n", [128, 1024, 4096, 16384])
+def test_p1_fft_vs_numpy_and_identities(n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    X = oracle.fft(x, -1)
+    # independent library routine (pocketfft), same sign convention exp(-2 pi i k n / N)
+    assert np.max(np.abs(X - np.fft.fft(x))) < 1e-9
+    # inverse(forward) = N * identity
+    assert np.max(np.abs(oracle.fft(X, +1) / n - x)) < 1e-12
+    # Parseval
+    assert abs(np.sum(np.abs(X) ** 2) / n - np.sum(np.abs(x) ** 2)) < 1e-8 * n
+    # delta -> flat spectrum of ones; delta at n0 -> exp(-2 pi i k n0 / N) (shift theorem)
+    d = np.zeros(n, complex); d[0] = 1
+    assert np.max(np.abs(oracle.fft(d, -1) - 1)) < 1e-13
+    n0 = 7
+    d = np.zeros(n, complex); d[n0] = 1
+    k = np.arange(n)
+    assert np.max(np.abs(oracle.fft(d, -1) - np.exp(-2j * np.pi * k * n0 / n))) < 1e-11
+    # linearity / transposed operand check: FFT of a pure tone is a single bin at +k0
+    k0 = 5
+    tone = np.exp(2j * np.pi * k0 * np.arange(n) / n)
+    T = oracle.fft(tone, -1)
+    assert abs(T[k0] - n) < 1e-8 and np.max(np.abs(np.delete(T, k0))) < 1e-8
+
+
+# ----------------------------------------------------------------------------- P2: chirp formula (Eq. 3)
+def test_p2_chirp_phase_matches_eq1_expansion_in_extended_precision():
+    """Eq. 1 -> Eq. 2 -> Eq. 3: the in-band term equals
+    D*DM*[1/(f_c+f) - 1/f_c + f/f_c^2] exactly; evaluated with 50 digits."""
+    mpmath.mp.dps = 50
+    for (dm, fc, f) in [(10.0, 317.125e6, -125e3), (71.0, 309.03125e6, 31.25e3 * 0.37),
+                        (107.5, 200.09765625e6, -97656.25), (150.0, 142.015625e6, 15625.0 * 0.99),
+                        (-26.77, 610e6, 1.0e3)]:
+        D, DM, FC, F = map(mpmath.mpf, (D_HZ, dm, fc, f))
+        ref = D * DM * (1 / (FC + F) - 1 / FC + F / FC ** 2)
+        got = oracle.chirp_phase_cycles(dm, fc, f)
+        assert abs(got - float(ref)) <= 1e-13 * max(1.0, abs(float(ref)))
+    assert oracle.chirp_phase_cycles(10.0, 325e6, 0.0) == 0.0
+    # psi >= 0 on both sides of the centre for DM > 0
+    assert oracle.chirp_phase_cycles(10.0, 325e6, -1e5) > 0 and oracle.chirp_phase_cycles(10.0, 325e6, 1e5) > 0
+
+
+def test_p2_chirp_array_unit_modulus_sign_and_bin_order():
+    cfg = cfg_tiny()
+    H = oracle.chirp(cfg, 0, 0)
+    assert abs(H[0] - 1.0) < 1e-15                       # f = 0 -> psi = 0
+    assert np.max(np.abs(np.abs(H) - 1.0)) < 1e-14       # no taper -> pure phase
+    dv = oracle.chan_width(cfg)
+    assert dv == 250e3
+    # bin order (R5): k < N/2 positive, N/2 -> -dv/2
+    assert oracle.bin_freq(cfg, 1) == dv / 1024 and oracle.bin_freq(cfg, 512) == -dv / 2
+    assert oracle.bin_freq(cfg, 1023) == -dv / 1024
+    # channel centres (R3): tile the band
+    assert oracle.chan_freq(cfg, 0) == 317e6 + 125e3 and oracle.chan_freq(cfg, 63) == 333e6 - 125e3
+    # sign (R1): +i, i.e. angle(H[k]) = +2 pi psi for small psi
+    k = 3
+    psi = float(mpmath.mpf(D_HZ) * 10 * mpmath.mpf(oracle.bin_freq(cfg, k)) ** 2
+                / ((oracle.chan_freq(cfg, 0) + oracle.bin_freq(cfg, k)) * oracle.chan_freq(cfg, 0) ** 2))
+    assert 0 < psi < 0.25
+    assert abs(np.angle(H[k]) - 2 * np.pi * psi) < 1e-12
+    # independent full-array evaluation with mpmath at a few bins, including large phases
+    mpmath.mp.dps = 40
+    fc = mpmath.mpf(oracle.chan_freq(cfg, 0))
+    for k in (100, 511, 512, 700, 1023):
+        f = mpmath.mpf(oracle.bin_freq(cfg, k))
+        ph = 2 * mpmath.pi * mpmath.mpf(D_HZ) * 10 * f ** 2 / ((fc + f) * fc ** 2)
+        ref = complex(mpmath.cos(ph), mpmath.sin(ph))
+        assert abs(H[k] - ref) < 1e-11
+
+
+def test_p2_tapers():
+    dv = 62.5e3
+    assert oracle.taper("none", 1234.0, dv) == 1.0
+    assert abs(oracle.taper("hann", 0.0, dv) - 1.0) < 1e-15 and abs(oracle.taper("hann", dv / 4, dv) - 0.5) < 1e-15
+    assert abs(oracle.taper("hann", -dv / 2, dv)) < 1e-30
+    assert oracle.taper("welch", 0.0, dv) == 1.0 and abs(oracle.taper("welch", dv / 4, dv) - 0.75) < 1e-15
+    assert oracle.taper("welch", -dv / 2, dv) == 0.0
+    # mean(w^2) over the band: 3/8 (Hann), 8/15 (Welch)
+    f = (np.arange(4096) - 2048) / 4096 * dv
+    assert abs(np.mean([oracle.taper("hann", x, dv) ** 2 for x in f]) - 0.375) < 1e-3
+    assert abs(np.mean([oracle.taper("welch", x, dv) ** 2 for x in f]) - 8 / 15) < 1e-3
+
+
+# ----------------------------------------------------------------------------- P3: delay law and constant D
+def test_p3_group_delay_is_the_cold_plasma_delay():
+    """-dpsi/df must be D*DM*(1/(f_c+f)^2 - 1/f_c^2): the textbook dispersion delay
+    4.148808 ms * DM * (f/GHz)^-2 relative to the channel centre."""
+    dm, fc = 57.0, 320.0e6
+    for f in (-30e3, -1e3, 2e3, 31e3):
+        h = 1.0
+        dpsi = (oracle.chirp_phase_cycles(dm, fc, f + h) - oracle.chirp_phase_cycles(dm, fc, f - h)) / (2 * h)
+        t_ms = lambda fr: 4.148808 * dm * (fr / 1e9) ** -2      # ms
+        ref = (t_ms(fc + f) - t_ms(fc)) * 1e-3                   # s, arrival(f_c+f) - arrival(f_c)
+        assert abs(-dpsi - ref) < 1e-6 * abs(ref)
+    # in-band smear
+    lo, hi = 317e6, 317.25e6
+    assert abs(oracle.smear_seconds(10.0, lo, hi) - 4.148808e-3 * 10 * ((lo / 1e9) ** -2 - (hi / 1e9) ** -2)) < 1e-15
+
+
+def test_p3_filter_delays_low_edge_advances_high_edge():
+    """Sign bookkeeping of R1/R9: tau(f) = -dpsi/df > 0 (delay) below centre, < 0 above, for DM > 0."""
+    dm, fc, h = 10.0, 317.125e6, 1.0
+    tau = lambda f: -(oracle.chirp_phase_cycles(dm, fc, f + h) - oracle.chirp_phase_cycles(dm, fc, f - h)) / (2 * h)
+    assert tau(-100e3) > 0 and tau(+100e3) < 0
+    assert tau(-100e3) > -tau(+100e3)          # the low side is the longer one (1/f^2 law)
+
+
+# ----------------------------------------------------------------------------- P4: numbers the paper prints
+@pytest.mark.parametrize("fc_mhz,bw_mhz,key", [(610, 16, "MAXDM_610_16"), (610, 32, "MAXDM_610_32"),
+                                               (325, 16, "MAXDM_325_16"), (325, 32, "MAXDM_325_32")])
+def test_p4_max_dm_figures_map_to_one_transform_length(fc_mhz, bw_mhz, key):
+    """the four largest DMs that fit the 6 GB card.  With the smear function and the
+    N rule of P:L139-141 (real Nyquist sampling, 2*BW samples/s) all four must give N = 2^27,
+    and a DM 20 % larger must need 2^28 (so they really are the maxima)."""
+    dm = GOLD[key]
+    lo, hi = (fc_mhz - bw_mhz / 2) * 1e6, (fc_mhz + bw_mhz / 2) * 1e6
+    fs = 2 * bw_mhz * 1e6
+    assert oracle.nfft_rule(oracle.smear_seconds(dm, lo, hi) * fs) == 2 ** 27
+    assert oracle.nfft_rule(oracle.smear_seconds(1.2 * dm, lo, hi) * fs) == 2 ** 28
+
+
+def test_p4_nfft_rule_boundaries():
+    assert oracle.nfft_rule(100.0) == 256          # smallest power of 2 GREATER than 200
+    assert oracle.nfft_rule(128.0) == 512          # 2*128 = 256 is not greater than 256
+    assert oracle.nfft_rule(0.3) == 1
+
+
+def test_p4_data_rates_and_time_resolution():
+    """120 / 240 / 1500 GB/h at 16 / 32 / 200 MHz pins 2 bytes per complex channel sample at a
+    total rate of BW complex samples/s; P:L35 / P:L99: 256 channels over 16 MHz -> 62.5 kHz -> 16 us."""
+    for bw, key in ((16e6, "RATE_16MHZ_GB_H"), (32e6, "RATE_32MHZ_GB_H"), (200e6, "RATE_200MHZ_GB_H")):
+        gb_h = bw * 2 * 3600 / 1e9
+        assert abs(gb_h - GOLD[key]) / GOLD[key] < 0.05
+    c16 = oracle.OracleConfig(256, 16e6, 325e6, (1.0,), 2048, 8)
+    assert oracle.chan_width(c16) == GOLD["CHANW_16MHZ_KHZ"] * 1e3
+    assert abs(1e6 / oracle.chan_width(c16) - GOLD["TRES_256CH_US"]) < 1e-9
+    c32 = oracle.OracleConfig(256, 32e6, 325e6, (1.0,), 2048, 8)
+    assert oracle.chan_width(c32) == GOLD["CHANW_32MHZ_KHZ"] * 1e3
+    c512 = oracle.OracleConfig(512, 16e6, 325e6, (1.0,), 2048, 8)
+    assert abs(1e6 / oracle.chan_width(c512) - GOLD["TRES_512CH_US"]) < 1e-9
+
+
+# ----------------------------------------------------------------------------- P5: impulse response support
+def test_p5_impulse_response_support_and_scaling():
+    """'The length of the response is equal to the dispersion time in the observing band';
+    P:L45: length ~ f^-3, ~ DM, ~ BW^2."""
+    cfg = cfg_tiny()
+    head, tail, L = oracle.framing(cfg)
+    H = oracle.chirp(cfg, 0, 0)
+    h = np.fft.ifft(H)                       # lag m at index m (m >= 0) or N+m (m < 0)
+    e = np.abs(h) ** 2
+    inside = e[: head + 1].sum() + e[len(e) - tail:].sum()
+    assert inside / e.sum() > 0.99
+    # energy really is spread over ~ the smear (not concentrated): 10 % of the support holds < 50 %
+    assert e[:8].sum() + e[-8:].sum() < 0.5 * e.sum()
+
+    def smear(fc, dm, dv):
+        return oracle.smear_seconds(dm, fc - dv / 2, fc + dv / 2) * dv
+    s0 = smear(317.125e6, 10.0, 250e3)
+    assert abs(s0 - 162.6) < 0.2                                             # 162.6 samples
+    assert abs(smear(317.125e6, 20.0, 250e3) / s0 - 2.0) < 1e-9              # ~ DM^1
+    assert abs(smear(317.125e6, 10.0, 500e3) / s0 - 4.0) < 0.01              # ~ BW^2
+    assert abs(smear(2 * 317.125e6, 10.0, 250e3) / s0 - 2.0 ** GOLD["SCALE_FREQ_EXP"]) < 0.001   # ~ f^-3
+
+
+@pytest.mark.parametrize("name,expect", [("tiny", (96, 96, 832, 74)), ("gmrt16", (32, 32, 1984, 251)),
+                                         ("gmrt32", (40, 56, 4000, 249)), ("lowfreq", (224, 224, 15936, 31)),
+                                         ("wideband", (2176, 2176, 12032, 129))])
+def test_p5_framing_of_the_five_workloads(name, expect):
+    """R9 framing; BASELINE configs[0]: 'overlap = per-channel smear samples rounded up to a multiple
+    of 32' -> 192 / 64 / 96 / 448 for configs 1-4."""
+    w = datagen.WORKLOADS[name]
+    cfg = oracle.OracleConfig(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
+    head, tail, L = oracle.framing(cfg)
+    assert (head, tail, L, oracle.n_blocks(cfg, w.n_samp)) == expect
+    assert head % w.n_int == 0 and L % w.n_int == 0 and head + tail + L == w.n_fft
+    dv = w.chan_width_hz
+    lo = w.f_center_hz - w.bw_hz / 2
+    smear = oracle.smear_seconds(max(w.dm_trials), lo, lo + dv) * dv
+    if name != "wideband":
+        assert head + tail == 32 * math.ceil(smear / 32) or head + tail == 32 * math.ceil((smear + 2) / 32)
+    assert head + tail >= smear
+
+
+def test_p5_framing_negative_dm_swaps_head_and_tail():
+    a = oracle.framing(cfg_tiny(dm=(10.0,), n_int=1))
+    b = oracle.framing(cfg_tiny(dm=(-10.0,), n_int=1))
+    assert a[0] + a[1] == b[0] + b[1]
+    assert a[0] > a[1] - 32 and b[0] <= a[1] and b[1] >= a[0]
+    with pytest.raises(ValueError):
+        oracle.framing(cfg_tiny(dm=(100.0,)))       # smear 1626 samples > N = 1024
+
+
+# ----------------------------------------------------------------------------- helpers for P6-P13
+def _to_int8(z):
+    """complex array [T][C] -> int8 [T][C][2]; asserts exact representability is NOT required."""
+    v = np.stack([np.rint(z.real), np.rint(z.imag)], axis=-1)
+    assert np.max(np.abs(v)) <= 127
+    return v.astype(np.int8)
+
+
+def _whole_series_filter(x, dm, fc, dv, sign):
+    """ONE long transform over the whole series (numpy FFT): multiply by exp(sign * 2 pi i psi)."""
+    n = x.size
+    f = np.fft.fftfreq(n, d=1.0 / dv)
+    psi = D_HZ * dm * f * f / ((fc + f) * fc * fc)
+    return np.fft.ifft(np.fft.fft(x) * np.exp(sign * 2j * np.pi * psi))
+
+
+# ----------------------------------------------------------------------------- P6: chirp o inverse chirp
+def test_p6_chirp_times_inverse_chirp_is_identity():
+    """north_star identity: applying chirp then inverse chirp returns the input.  H(DM) * H(-DM) = 1."""
+    cp = cfg_tiny(dm=(10.0, -10.0), n_int=1)
+    H1, H2 = oracle.chirp(cp, 0, 5), oracle.chirp(cp, 1, 5)
+    assert np.max(np.abs(H1 * H2 - 1.0)) < 1e-12
+    assert np.max(np.abs(H2 - np.conj(H1))) < 1e-12
+    rng = np.random.default_rng(6)
+    x = rng.standard_normal(1024) + 1j * rng.standard_normal(1024)
+    y = oracle.fft(oracle.fft(x, -1) * H1, +1) / 1024
+    z = oracle.fft(oracle.fft(y, -1) * H2, +1) / 1024
+    assert np.max(np.abs(z - x)) < 1e-12
+
+
+# ----------------------------------------------------------------------------- P7: normalisation / noise power
+def test_p7_white_noise_power_is_preserved():
+    """north_star identity: output intensity for white noise matches the input power.
+    int8 Gaussian sigma=20 per component, rounded: E|x|^2 = 2*(sigma^2 + 1/12) = 800.17;
+    unitary filter + 1/N inverse (R7) -> mean(out) = n_int * 800.17."""
+    cfg = cfg_tiny(n_chan=8, bw_hz=2e6, f_center_hz=318e6)
+    x = datagen.noise_only(40000, 8, seed=7)
+    out = oracle.dedisp(cfg, x, n_threads=4)
+    expect = cfg.n_int * 2 * (20.0 ** 2 + 1 / 12)
+    n_indep = out.size * cfg.n_int
+    assert abs(out.mean() / expect - 1.0) < 5.0 / math.sqrt(n_indep)
+    # and it matches the integer input power over the same rows to sampling error
+    assert abs(out.mean() / (cfg.n_int * np.mean(np.sum(x.astype(np.float64) ** 2, axis=-1))) - 1.0) < 1e-2
+
+
+# ----------------------------------------------------------------------------- P8: DM = 0 closed form
+@pytest.mark.parametrize("n_fft,n_int,C,T", [(64, 4, 3, 1000), (128, 8, 2, 1111), (1024, 16, 4, 5000)])
+def test_p8_dm_zero_is_integer_boxcar_power(n_fft, n_int, C, T):
+    """DM = 0 -> H = 1 -> the whole path is the identity, so out[j] must equal the INTEGER
+    sum of re^2 + im^2 over rows head + j*n_int .. (a textbook boxcar), across every block boundary.
+    Pins unpack, [t][chan][2] layout, framing, block stitching, 1/N, detection, integration."""
+    cfg = oracle.OracleConfig(C, 1e6, 300e6, (0.0,), n_fft, n_int)
+    head, tail, L = oracle.framing(cfg)
+    assert (head, tail, L) == (0, 0, n_fft)
+    x = datagen.uniform_int8(T, C, seed=8)          # includes -128
+    out = oracle.dedisp(cfg, x)
+    nb = T // n_fft
+    assert out.shape == (1, C, nb * n_fft // n_int) and nb >= 2
+    p = np.sum(x.astype(np.int64) ** 2, axis=-1)    # [T][C]
+    ref = p[: nb * n_fft].reshape(-1, n_int, C).sum(axis=1).T
+    assert np.max(np.abs(out[0] - ref)) < 1e-7 * ref.max()
+
+
+def test_p8_nonzero_head_boxcar_with_dm_pair():
+    """Same closed form with head, tail > 0: a plan whose two trial DMs are (+dm, 0): the DM = 0 row
+    must be the boxcar of rows head + j*n_int (R12) even though the framing comes from the other DM."""
+    cfg = cfg_tiny(n_chan=2, bw_hz=0.5e6, f_center_hz=317.25e6, dm=(10.0, 0.0))
+    head, tail, L = oracle.framing(cfg)
+    assert head > 0 and tail > 0
+    x = datagen.uniform_int8(5000, 2, seed=9)
+    out = oracle.dedisp(cfg, x)
+    nb = (5000 - head - tail) // L
+    p = np.sum(x.astype(np.int64) ** 2, axis=-1)
+    ref = p[head: head + nb * L].reshape(-1, cfg.n_int, 2).sum(axis=1).T
+    assert out.shape[2] == nb * L // cfg.n_int
+    assert np.max(np.abs(out[1] - ref)) < 1e-7 * ref.max()
+    assert np.max(np.abs(out[0] - ref)) > 1e-3 * ref.max()      # the DM = 10 row is NOT the boxcar
+
+
+# ----------------------------------------------------------------------------- P9: delta collapses, discard placement
+@pytest.mark.parametrize("dm", [10.0, -10.0])
+def test_p9_dispersed_delta_collapses_to_a_delta(dm):
+    """north_star identity: a delta pulse dispersed at DM collapses back to a delta when dedispersed at
+    the same DM.  The delta is dispersed with conj(H) through ONE whole-series numpy FFT (independent of
+    the block framing), quantised to int8, then run through the block algorithm with n_int = 1.
+    Deltas sit mid-block, at the last valid sample of block 0 and at the first valid sample of block 1:
+    a wrong head/tail split or a wrong chirp sign smears or loses them."""
+    cfg = cfg_tiny(n_chan=1, bw_hz=250e3, f_center_hz=317.125e6, dm=(dm,), n_int=1)
+    head, tail, L = oracle.framing(cfg)
+    T = 3 * L + head + tail
+    fc, dv = oracle.chan_freq(cfg, 0), oracle.chan_width(cfg)
+    A = 700.0
+    spots = [head + L // 2, head + L - 1, head + L, head + 2 * L + 7]
+    x = np.zeros(T, complex)
+    for s in spots:
+        x[s] = A
+    xd = _whole_series_filter(x, dm, fc, dv, sign=-1)           # disperse = conj of the applied chirp
+    assert np.max(np.abs(xd)) < 127
+    out = oracle.dedisp(cfg, _to_int8(xd[:, None]))[0, 0]
+    assert out.size == 3 * L
+    tot = out.sum()
+    peak = sum(out[s - head] for s in spots)
+    assert peak / tot > 0.999
+    for s in spots:
+        assert abs(out[s - head] / A ** 2 - 1.0) < 0.02
+    # negative control: the opposite chirp sign does NOT collapse it
+    cfg_wrong = cfg_tiny(n_chan=1, bw_hz=250e3, f_center_hz=317.125e6, dm=(-dm,), n_int=1)
+    h2, t2, L2 = oracle.framing(cfg_wrong)
+    out_w = oracle.dedisp(cfg_wrong, _to_int8(xd[:, None]))[0, 0]
+    assert out_w.max() < 0.05 * A ** 2
+
+
+def test_p9_misplaced_discard_fails_visibly():
+    """If the valid window were taken at the wrong place (all the discard at one end) the collapsed
+    delta next to a block edge would lose energy: check with the voltage output of a unit."""
+    cfg = cfg_tiny(n_chan=1, bw_hz=250e3, f_center_hz=317.125e6, dm=(10.0,), n_int=1)
+    head, tail, L = oracle.framing(cfg)
+    fc, dv = oracle.chan_freq(cfg, 0), oracle.chan_width(cfg)
+    T = 2 * L + head + tail
+    x = np.zeros(T, complex)
+    x[head] = 700.0                                           # first valid sample of block 0
+    xd = _whole_series_filter(x, 10.0, fc, dv, sign=-1)
+    xi = _to_int8(xd[:, None])
+    out, volt = oracle.dedisp_units(cfg, xi, [0], [0], want_voltage=True)
+    assert abs(volt[0, 0, 0]) ** 2 / 700.0 ** 2 > 0.98
+    # emulate "discard everything at the beginning" (textbook wording P:L125): the block would then
+    # start head+tail rows later and the sample `head` of the series would fall in the discarded part;
+    # emulate "discard everything at the end": sample index 0 of a block needs `head` past samples that
+    # the block does not contain -> the same delta placed at block-local index 0 does not collapse.
+    x2 = np.zeros(T, complex); x2[0] = 700.0
+    xd2 = _whole_series_filter(x2, 10.0, fc, dv, sign=-1)
+    blk = np.fft.ifft(np.fft.fft(np.rint(xd2[:1024].real) + 1j * np.rint(xd2[:1024].imag)) * oracle.chirp(cfg, 0, 0))
+    assert abs(blk[0]) ** 2 / 700.0 ** 2 < 0.9                # polluted by the circular wrap
+
+
+# ----------------------------------------------------------------------------- P11: multi-DM rows
+def test_p11_multi_dm_rows_equal_single_dm_plans_when_framing_is_shared():
+    dms = (8.0, 9.0, 10.0)
+    kw = dict(n_chan=3, bw_hz=0.75e6, f_center_hz=317.375e6)
+    x = datagen.noise_only(6000, 3, seed=11)
+    multi = oracle.dedisp(cfg_tiny(dm=dms, **kw), x)
+    # the largest DM fixes the framing; add it as a second trial so single-DM plans share it
+    for i, dm in enumerate(dms):
+        single = oracle.dedisp(cfg_tiny(dm=(dm, dms[-1]), **kw), x)
+        assert np.array_equal(single[0], multi[i])
+
+
+# ----------------------------------------------------------------------------- P12: brute force on tiny inputs
+@pytest.mark.parametrize("n_fft", [64, 128])
+def test_p12_bruteforce_time_domain_circular_convolution(n_fft):
+    """Tiny case: per block, y[n] = sum_m h[m] x[(n-m) mod N] with h = IDFT(H) written out as loops;
+    H from the formula in mpmath; keep [head, N-tail); |.|^2; sums of n_int = 2."""
+    C, n_int, T = 2, 2, 5 * n_fft + 3
+    cfg = oracle.OracleConfig(C, 0.2e6, 100e6, (0.02,), n_fft, n_int)
+    head, tail, L = oracle.framing(cfg)
+    assert head > 0 and tail > 0 and L > 0
+    x = datagen.uniform_int8(T, C, seed=12)
+    out = oracle.dedisp(cfg, x)
+    nb = (T - head - tail) // L
+    mpmath.mp.dps = 30
+    dv = 0.1e6
+    for c in range(C):
+        fc = 100e6 - 0.1e6 + (c + 0.5) * dv
+        H = np.zeros(n_fft, complex)
+        for k in range(n_fft):
+            f = (k if k < n_fft // 2 else k - n_fft) * dv / n_fft
+            ph = 2 * mpmath.pi * mpmath.mpf(D_HZ) * mpmath.mpf("0.02") * mpmath.mpf(f) ** 2 / (
+                (mpmath.mpf(fc) + f) * mpmath.mpf(fc) ** 2)
+            H[k] = complex(mpmath.cos(ph), mpmath.sin(ph))
+        h = np.array([sum(H[k] * np.exp(2j * np.pi * k * m / n_fft) for k in range(n_fft)) / n_fft
+                      for m in range(n_fft)])
+        ref = []
+        for b in range(nb):
+            xb = x[b * L: b * L + n_fft, c, 0].astype(float) + 1j * x[b * L: b * L + n_fft, c, 1].astype(float)
+            y = np.array([sum(h[m] * xb[(n - m) % n_fft] for m in range(n_fft)) for n in range(n_fft)])
+            p = np.abs(y[head: head + L]) ** 2
+            ref.append(p.reshape(-1, n_int).sum(axis=1))
+        ref = np.concatenate(ref)
+        assert out.shape[2] == ref.size
+        assert np.max(np.abs(out[0, c] - ref)) < 1e-9 * ref.max()
+
+
+# ----------------------------------------------------------------------------- P13: tones and tapers
+@pytest.mark.parametrize("taper,k_frac,w", [("none", 0.25, 1.0), ("hann", 0.25, 0.5), ("welch", 0.25, 0.75),
+                                            ("hann", 0.5, 0.0), ("welch", 0.5, 0.0), ("hann", 0.0, 1.0),
+                                            ("welch", 0.75, 0.75)])
+def test_p13_exact_int8_tones(taper, k_frac, w):
+    """x[n] = A e^{2 pi i k0 n / N}, k0 in {0, N/4, N/2, 3N/4} is exactly representable in int8; a tone
+    sits in one FFT bin so out = n_int * A^2 * w(f_k0)^2 for ANY DM (|H| = w)."""
+    cfg = cfg_tiny(n_chan=2, bw_hz=0.5e6, f_center_hz=317.25e6, taper=taper)
+    head, tail, L = oracle.framing(cfg)
+    T, A = 4000, 100
+    n = np.arange(T)
+    z = A * np.exp(2j * np.pi * k_frac * n)
+    x = _to_int8(np.stack([z, z], axis=1))
+    out = oracle.dedisp(cfg, x)
+    expect = cfg.n_int * A * A * w * w
+    assert np.max(np.abs(out - expect)) < 1e-6 * (A * A * cfg.n_int)
+
+
+# ----------------------------------------------------------------------------- P14: science sanity on the tiny workload
+def test_p14_injected_pulsar_is_sharpest_at_its_dm():
+    """Statistical, not parity: fold the tiny workload's outputs at the injected period; the profile peak
+    is highest at the injected DM (10), lower at 5, lowest at 0; off-pulse level = n_int * 800.17."""
+    w = datagen.WORKLOADS["tiny"]
+    chans = [0, 31, 63]
+    x = datagen.generate(w, chans=chans)
+    fcs = datagen.chan_freqs_hz(w)
+    peaks = {}
+    for dm in (10.0, 5.0, 0.0):
+        tops = []
+        for i, c in enumerate(chans):
+            # single-channel plan centred on channel c with the same channel width
+            cfg = oracle.OracleConfig(1, w.chan_width_hz, float(fcs[c]), (dm, 10.0), w.n_fft, w.n_int)
+            head, tail, L = oracle.framing(cfg)
+            out = oracle.dedisp(cfg, np.ascontiguousarray(x[:, i:i + 1, :]))[0, 0]
+            t = (head + np.arange(out.size) * w.n_int + 0.5 * w.n_int) / w.chan_width_hz
+            delay = datagen.D_HZ2_S * w.pulse_dm * (1 / fcs[c] ** 2 - 1 / (w.f_center_hz + w.bw_hz / 2) ** 2)
+            ph = np.mod(t - delay, w.pulse_period_s) / w.pulse_period_s
+            nbin = 39
+            b = np.minimum((ph * nbin).astype(int), nbin - 1)
+            prof = np.bincount(b, out, nbin) / np.maximum(np.bincount(b, None, nbin), 1)
+            tops.append(prof.max())
+            if dm == 10.0:
+                assert abs(np.median(prof) / (w.n_int * 800.17) - 1.0) < 0.02
+                assert prof.argmax() == 0
+        peaks[dm] = np.mean(tops)
+    assert peaks[10.0] > 1.3 * peaks[5.0] > 1.3 * 1.2 * peaks[0.0]
