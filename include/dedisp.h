@@ -1,0 +1,135 @@
+/*
+ * dedisp.h -- C ABI of libdedisp: channelised overlap-save coherent dedispersion on one B200 (sm_100a).
+ *
+ * The operation is the data-parallel hot path of De & Gupta, "A Real-time Coherent Dedispersion Pipeline
+ * for the GMRT" (arXiv:1509.00186).  Citations "P:L<n>" are line numbers of the paper text;
+ * "R<n>" are the readings listed in DESIGN.md where the paper is silent or ambiguous.
+ *
+ * What one dedisp_execute() call computes, for every frequency channel c, overlap-save block b and trial DM d
+ * (stage order of P:L139-145 Fig. 4):
+ *   1. unpack   x[n] = (float)in[b*L+n][c].re + i*(float)in[b*L+n][c].im,  n in [0,N)      (R10)
+ *   2. forward  S[k] = sum_n x[n] exp(-2*pi*i*k*n/N)
+ *   3. chirp    Y[k] = S[k] * w(f_k) * exp(+2*pi*i*psi),  psi = D*DM_d*f_k^2/(f_c^2*(f_c+f_k)) (Eq. 3)
+ *               D = 4.148808e15 Hz^2 s / (pc cm^-3), f_c = F - B/2 + (c+1/2)*B/C,
+ *               f_k = k*dv/N (k < N/2) or (k-N)*dv/N, dv = B/C
+ *   4. inverse  y[n] = (1/N) sum_k Y[k] exp(+2*pi*i*k*n/N)                                    (R7)
+ *   5. discard  keep n in [head, head+L), L = N - head - tail                                (R9)
+ *   6. detect + integrate  out[d][c][b*L/n_int + j] = sum_{i<n_int} |y[head + j*n_int + i]|^2 (R11)
+ *
+ * Pointers: every pointer argument says HOST or DEVICE.  The library never takes ownership of caller buffers.
+ * Errors:   every call returns DEDISP_OK (0) or a negative DEDISP_E* code; no exceptions, no aborts, no output.
+ * Threads:  a plan may be used from one host thread at a time.
+ */
+#ifndef DEDISP_H
+#define DEDISP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dedisp_plan_s* dedisp_plan_t; /* opaque, owned by the library */
+
+enum {
+    DEDISP_OK = 0,
+    DEDISP_EINVAL = -1, /* bad argument (see each call) */
+    DEDISP_ENOMEM = -2, /* host or device allocation failed */
+    DEDISP_ECUDA = -3,  /* a CUDA call failed; dedisp_last_cuda_error() gives the cudaError_t */
+    DEDISP_ESHORT = -4, /* n_samp shorter than one block (n_fft samples) */
+    DEDISP_ENODEV = -5  /* no sm_100 device / no CUDA driver */
+};
+
+/* flags of dedisp_plan(): taper of the chirp function (P:L123 names Hanning and Welch; R6 gives the formulas) */
+enum {
+    DEDISP_TAPER_NONE = 0u,  /* w = 1 (default) */
+    DEDISP_TAPER_HANN = 1u,  /* w = cos^2(pi f/dv) */
+    DEDISP_TAPER_WELCH = 2u, /* w = 1 - (2f/dv)^2 */
+    DEDISP_TAPER_MASK = 3u
+};
+
+typedef struct {
+    int n_chan, n_dm, n_fft, n_int; /* echo of the arguments */
+    int head, tail, L;              /* overlap-save framing in use (R9): block b reads rows b*L .. b*L+N-1 */
+    double chan_width_hz;           /* dv = bw / n_chan = complex sample rate of one channel */
+    double max_smear_samples;       /* largest in-band dispersion time over channels and DMs, in samples */
+    int nfft_rule;                  /* smallest power of 2 > 2*max_smear_samples (advisory) */
+} dedisp_info_t;
+
+/*
+ * Overlap-save framing (pure host arithmetic, no GPU needed).  P:L121/L145: the number of samples to discard is the
+ * impulse-response length = dispersion time in the band.  R9: with the channel-centre reference the applied filter
+ * delays the low edge (needs `head` past samples) and advances the high edge (needs `tail` future samples); one
+ * framing for all channels and DMs:  head = roundup(n_del, n_int), head+tail = roundup(head+n_adv, lcm(32,n_int)).
+ *   dm: HOST array [n_dm], pc cm^-3, negative allowed (conjugate chirp; head/tail roles swap).
+ * Returns DEDISP_EINVAL if an argument is non-positive, F - B/2 <= 0, head+tail >= n_fft or L % n_int != 0.
+ */
+int dedisp_framing(int n_chan, double bw_hz, double f_center_hz, const double* dm, int n_dm, int n_fft, int n_int,
+                   int* head, int* tail, int* L);
+
+/*
+ * Create a plan on the current CUDA device: validates, computes the framing, builds the chirp table
+ * float2 [n_dm][n_chan][n_fft] (phase in fp64, value rounded to fp32, pre-scaled by 1/n_fft) and the FFT twiddles.
+ *   n_fft: one of 1024, 2048, 4096, 8192, 16384 (the built kernel sizes).  dm: HOST array, copied.
+ * Synchronises the device once.  Errors: EINVAL, ENOMEM, ECUDA, ENODEV.
+ */
+int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, double f_center_hz, const double* dm, int n_dm,
+                int n_fft, int n_int, unsigned flags);
+
+int dedisp_get_info(dedisp_plan_t plan, dedisp_info_t* info);
+
+/* Outputs per (dm, channel) of a one-shot call on n_samp samples per channel: nb*L/n_int with
+ * nb = floor((n_samp - head - tail)/L) (R12: no zero padding, trailing partial block dropped); 0 if too short. */
+long long dedisp_out_samples(dedisp_plan_t plan, long long n_samp);
+
+/* Pre-size the plan's device scratch (the channel-major int8 copy of the input) for calls of up to n_samp samples,
+ * so that dedisp_execute never allocates.  Synchronises the device if it has to grow. */
+int dedisp_reserve(dedisp_plan_t plan, long long n_samp);
+
+/*
+ * Enqueue steps 1-6 on `cuda_stream` (a cudaStream_t; NULL = legacy default stream).  Never synchronises unless the
+ * scratch has to grow (see dedisp_reserve).  Results are valid once the caller has synchronised the stream.
+ *   d_in   DEVICE, int8 [n_samp][n_chan][2] time-major, re then im (R10); 2-byte aligned; read only.
+ *   d_out  DEVICE, float [n_dm][n_chan][out_stride]; the first dedisp_out_samples() entries of each row are written.
+ * Errors: EINVAL (null pointer, out_stride too small), ESHORT, ENOMEM, ECUDA.
+ */
+int dedisp_execute(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, float* d_out, long long out_stride,
+                   void* cuda_stream);
+
+/*
+ * Streaming form (host->device copy, compute and device->host copy overlapped on three streams; P:L270:
+ * the samples lost at a block edge are prefixed to the next block).  Push consecutive chunks of the same observation;
+ * the plan keeps the unconsumed tail on the device so that the concatenated output equals a one-shot call on the
+ * concatenated input (R12).
+ *   h_in   HOST (pinned for overlap), int8 [n_samp][n_chan][2].
+ *   h_out  HOST (pinned), float [n_dm][n_chan][out_stride]: receives the outputs completed by THIS chunk in columns
+ *          [0, *n_out); valid after dedisp_stream_sync().
+ * The call returns after enqueueing; h_in must stay untouched until the next push or sync returns.
+ */
+int dedisp_stream_begin(dedisp_plan_t plan, long long max_chunk_samp);
+int dedisp_stream_push(dedisp_plan_t plan, const int8_t* h_in, long long n_samp, float* h_out, long long out_stride,
+                       long long* n_out);
+int dedisp_stream_sync(dedisp_plan_t plan);
+int dedisp_stream_end(dedisp_plan_t plan);
+
+int dedisp_destroy(dedisp_plan_t plan);
+
+const char* dedisp_strerror(int code);
+int dedisp_last_cuda_error(void); /* cudaError_t of the last DEDISP_ECUDA on this thread */
+
+/*
+ * Test hooks (used by the parity tests only).
+ * dedisp_debug_unpack: the framed, unpacked block (step 1) of (chan, block) as float [n_fft][2] on the DEVICE.
+ * dedisp_debug_chirp:  copies the chirp table row (d, chan) to HOST as float [n_fft][2] (includes the 1/n_fft scale).
+ * dedisp_debug_voltage: steps 1-5 for one (chan, block): DEVICE float [n_dm][L][2] dedispersed complex voltages.
+ */
+int dedisp_debug_unpack(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, int chan, long long block,
+                        float* d_block, void* cuda_stream);
+int dedisp_debug_chirp(dedisp_plan_t plan, int d, int chan, float* h_chirp);
+int dedisp_debug_voltage(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, int chan, long long block,
+                         float* d_volt, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEDISP_H */

@@ -1,0 +1,196 @@
+"""ctypes binding of libdedisp (include/dedisp.h).  Argument marshalling only: every step of the path runs in the
+library's CUDA kernels.  There is no CPU fallback: if the library is missing or fails to load, importing raises."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Sequence
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libdedisp.so")
+
+OK, EINVAL, ENOMEM, ECUDA, ESHORT, ENODEV = 0, -1, -2, -3, -4, -5
+TAPER = {"none": 0, "hann": 1, "welch": 2}
+
+# every symbol include/dedisp.h declares (tests check that the library exports all of them)
+SYMBOLS = (
+    "dedisp_framing", "dedisp_plan", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
+    "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_destroy",
+    "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
+)
+
+
+class Info(C.Structure):
+    _fields_ = [("n_chan", C.c_int), ("n_dm", C.c_int), ("n_fft", C.c_int), ("n_int", C.c_int),
+                ("head", C.c_int), ("tail", C.c_int), ("L", C.c_int),
+                ("chan_width_hz", C.c_double), ("max_smear_samples", C.c_double), ("nfft_rule", C.c_int)]
+
+
+class DedispError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = _lib.dedisp_strerror(code).decode()
+        if code == ECUDA:
+            msg += f" [cudaError {_lib.dedisp_last_cuda_error()}]"
+        super().__init__(f"{where}: {msg} ({code})")
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1509_00186_b200.build` "
+                          "(the CUDA library is the product; there is no fallback)")
+    L = C.CDLL(LIB_PATH)
+    dp, ip, vp, ll = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p, C.c_longlong
+    L.dedisp_framing.argtypes = [C.c_int, C.c_double, C.c_double, dp, C.c_int, C.c_int, C.c_int, ip, ip, ip]
+    L.dedisp_plan.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, dp, C.c_int, C.c_int, C.c_int, C.c_uint]
+    L.dedisp_get_info.argtypes = [vp, C.POINTER(Info)]
+    L.dedisp_out_samples.argtypes = [vp, ll]
+    L.dedisp_out_samples.restype = ll
+    L.dedisp_reserve.argtypes = [vp, ll]
+    L.dedisp_execute.argtypes = [vp, vp, ll, vp, ll, vp]
+    L.dedisp_stream_begin.argtypes = [vp, ll]
+    L.dedisp_stream_push.argtypes = [vp, vp, ll, vp, ll, C.POINTER(ll)]
+    L.dedisp_stream_sync.argtypes = [vp]
+    L.dedisp_stream_end.argtypes = [vp]
+    L.dedisp_destroy.argtypes = [vp]
+    L.dedisp_strerror.argtypes = [C.c_int]
+    L.dedisp_strerror.restype = C.c_char_p
+    L.dedisp_last_cuda_error.argtypes = []
+    L.dedisp_debug_unpack.argtypes = [vp, vp, ll, C.c_int, ll, vp, vp]
+    L.dedisp_debug_chirp.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.dedisp_debug_voltage.argtypes = [vp, vp, ll, C.c_int, ll, vp, vp]
+    return L
+
+
+_lib = _load()
+
+
+def lib() -> C.CDLL:
+    return _lib
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != OK:
+        raise DedispError(rc, where)
+
+
+def _dm_array(dm: Sequence[float]):
+    dm = [float(v) for v in dm]
+    return (C.c_double * len(dm))(*dm), len(dm)
+
+
+def dedisp_framing(n_chan: int, bw_hz: float, f_center_hz: float, dm: Sequence[float], n_fft: int, n_int: int):
+    """(head, tail, L) of the overlap-save framing; host arithmetic only (no GPU needed)."""
+    arr, n = _dm_array(dm)
+    h, t, l = C.c_int(), C.c_int(), C.c_int()
+    _check(_lib.dedisp_framing(n_chan, bw_hz, f_center_hz, arr, n, n_fft, n_int, C.byref(h), C.byref(t), C.byref(l)),
+           "dedisp_framing")
+    return h.value, t.value, l.value
+
+
+def dedisp_plan(n_chan: int, bw_hz: float, f_center_hz: float, dm: Sequence[float], n_fft: int, n_int: int,
+                taper: str = "none") -> "Plan":
+    return Plan(n_chan, bw_hz, f_center_hz, dm, n_fft, n_int, taper)
+
+
+class Plan:
+    """Owns a dedisp_plan_t.  Methods take torch tensors (or raw pointers) and pass pointers through."""
+
+    def __init__(self, n_chan, bw_hz, f_center_hz, dm, n_fft, n_int, taper="none"):
+        self._h = C.c_void_p()
+        arr, n = _dm_array(dm)
+        _check(_lib.dedisp_plan(C.byref(self._h), n_chan, bw_hz, f_center_hz, arr, n, n_fft, n_int, TAPER[taper]),
+               "dedisp_plan")
+        info = Info()
+        _check(_lib.dedisp_get_info(self._h, C.byref(info)), "dedisp_get_info")
+        self.info = info
+        self.n_chan, self.n_dm, self.n_fft, self.n_int = info.n_chan, info.n_dm, info.n_fft, info.n_int
+        self.head, self.tail, self.L = info.head, info.tail, info.L
+
+    # -- sizes ------------------------------------------------------------------------------------------------
+    def out_samples(self, n_samp: int) -> int:
+        return int(_lib.dedisp_out_samples(self._h, n_samp))
+
+    def n_blocks(self, n_samp: int) -> int:
+        return self.out_samples(n_samp) // (self.L // self.n_int)
+
+    def reserve(self, n_samp: int) -> None:
+        _check(_lib.dedisp_reserve(self._h, n_samp), "dedisp_reserve")
+
+    # -- one-shot ---------------------------------------------------------------------------------------------
+    def execute(self, d_in, d_out=None, stream=None):
+        """d_in: CUDA int8 tensor [n_samp][n_chan][2]; returns/fills CUDA float32 [n_dm][n_chan][n_out]."""
+        import torch
+        assert d_in.is_cuda and d_in.dtype == torch.int8 and d_in.is_contiguous()
+        assert d_in.dim() == 3 and d_in.shape[1] == self.n_chan and d_in.shape[2] == 2
+        n_samp = d_in.shape[0]
+        n_out = self.out_samples(n_samp)
+        if d_out is None:
+            d_out = torch.empty((self.n_dm, self.n_chan, max(n_out, 0)), dtype=torch.float32, device=d_in.device)
+        assert d_out.is_cuda and d_out.dtype == torch.float32 and d_out.is_contiguous()
+        assert d_out.dim() == 3 and d_out.shape[0] == self.n_dm and d_out.shape[1] == self.n_chan
+        st = torch.cuda.current_stream(d_in.device).cuda_stream if stream is None else stream
+        _check(_lib.dedisp_execute(self._h, d_in.data_ptr(), n_samp, d_out.data_ptr(), d_out.shape[2], st),
+               "dedisp_execute")
+        return d_out
+
+    def execute_ptr(self, in_ptr: int, n_samp: int, out_ptr: int, out_stride: int, stream: int = 0) -> None:
+        _check(_lib.dedisp_execute(self._h, in_ptr, n_samp, out_ptr, out_stride, stream), "dedisp_execute")
+
+    # -- streaming --------------------------------------------------------------------------------------------
+    def stream_begin(self, max_chunk_samp: int) -> None:
+        _check(_lib.dedisp_stream_begin(self._h, max_chunk_samp), "dedisp_stream_begin")
+
+    def stream_push(self, h_in, h_out) -> int:
+        """h_in: pinned int8 [n][C][2]; h_out: pinned float32 [n_dm][C][stride]; returns outputs written."""
+        n = C.c_longlong(0)
+        _check(_lib.dedisp_stream_push(self._h, h_in.data_ptr(), h_in.shape[0], h_out.data_ptr(), h_out.shape[2],
+                                       C.byref(n)), "dedisp_stream_push")
+        return int(n.value)
+
+    def stream_sync(self) -> None:
+        _check(_lib.dedisp_stream_sync(self._h), "dedisp_stream_sync")
+
+    def stream_end(self) -> None:
+        _check(_lib.dedisp_stream_end(self._h), "dedisp_stream_end")
+
+    # -- test hooks -------------------------------------------------------------------------------------------
+    def debug_unpack(self, d_in, chan: int, block: int):
+        import torch
+        out = torch.empty((self.n_fft, 2), dtype=torch.float32, device=d_in.device)
+        st = torch.cuda.current_stream(d_in.device).cuda_stream
+        _check(_lib.dedisp_debug_unpack(self._h, d_in.data_ptr(), d_in.shape[0], chan, block, out.data_ptr(), st),
+               "dedisp_debug_unpack")
+        return out
+
+    def debug_chirp(self, d: int, chan: int):
+        import numpy as np
+        h = np.empty((self.n_fft, 2), dtype=np.float32)
+        _check(_lib.dedisp_debug_chirp(self._h, d, chan, h.ctypes.data), "dedisp_debug_chirp")
+        return h[:, 0] + 1j * h[:, 1]
+
+    def debug_voltage(self, d_in, chan: int, block: int):
+        import torch
+        out = torch.empty((self.n_dm, self.L, 2), dtype=torch.float32, device=d_in.device)
+        st = torch.cuda.current_stream(d_in.device).cuda_stream
+        _check(_lib.dedisp_debug_voltage(self._h, d_in.data_ptr(), d_in.shape[0], chan, block, out.data_ptr(), st),
+               "dedisp_debug_voltage")
+        return out
+
+    # -- lifetime ---------------------------------------------------------------------------------------------
+    def destroy(self) -> None:
+        if self._h:
+            _lib.dedisp_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()

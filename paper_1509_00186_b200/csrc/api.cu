@@ -1,0 +1,207 @@
+// api.cu -- plan lifecycle and the one-shot execute of libdedisp (C ABI of include/dedisp.h).
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "dedisp_internal.h"
+
+extern "C" const char* dedisp_strerror(int code)
+{
+    switch (code) {
+        case DEDISP_OK: return "ok";
+        case DEDISP_EINVAL: return "invalid argument";
+        case DEDISP_ENOMEM: return "out of memory";
+        case DEDISP_ECUDA: return "CUDA error (see dedisp_last_cuda_error)";
+        case DEDISP_ESHORT: return "input shorter than one transform block";
+        case DEDISP_ENODEV: return "no usable sm_100 CUDA device";
+        default: return "unknown dedisp status";
+    }
+}
+
+extern "C" int dedisp_last_cuda_error(void) { return g_dedisp_last_cuda; }
+
+static void free_plan(dedisp_plan_s* p)
+{
+    if (!p) return;
+    dedisp_stream_free(p);
+    if (p->d_chirp) cudaFree(p->d_chirp);
+    if (p->d_twiddle) cudaFree(p->d_twiddle);
+    if (p->d_xt) cudaFree(p->d_xt);
+    if (p->d_spec) cudaFree(p->d_spec);
+    free(p->dm);
+    delete p;
+}
+
+extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, double f_center_hz, const double* dm,
+                           int n_dm, int n_fft, int n_int, unsigned flags)
+{
+    if (!out_plan) return DEDISP_EINVAL;
+    *out_plan = nullptr;
+    if ((flags & ~DEDISP_TAPER_MASK) || (flags & DEDISP_TAPER_MASK) == 3u) return DEDISP_EINVAL;
+    if (n_fft <= 0 || (n_fft & (n_fft - 1)) || !dedisp_fused_supported(n_fft)) return DEDISP_EINVAL;
+    int head, tail, L;
+    double smear = 0.0;
+    int rc = dedisp_framing_impl(n_chan, bw_hz, f_center_hz, dm, n_dm, n_fft, n_int, &head, &tail, &L, &smear);
+    if (rc != DEDISP_OK) return rc;
+
+    int dev = 0, n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) {
+        (void)cudaGetLastError();
+        return DEDISP_ENODEV;
+    }
+    DEDISP_CUDA_TRY(cudaGetDevice(&dev));
+    int major = 0;
+    DEDISP_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return DEDISP_ENODEV;  // the kernels are built for sm_100a only
+
+    dedisp_plan_s* p = new (std::nothrow) dedisp_plan_s();
+    if (!p) return DEDISP_ENOMEM;
+    memset(p, 0, sizeof(*p));
+    p->n_chan = n_chan; p->n_dm = n_dm; p->n_fft = n_fft; p->n_int = n_int;
+    p->bw_hz = bw_hz; p->f_center_hz = f_center_hz; p->flags = flags;
+    p->head = head; p->tail = tail; p->L = L; p->device = dev;
+    p->max_smear_samples = smear;
+    {   // P:L139-141 length rule, advisory
+        long long n = 1;
+        while ((double)n <= 2.0 * smear && n < (1ll << 30)) n <<= 1;
+        p->nfft_rule = (int)n;
+    }
+    p->dm = (double*)malloc(sizeof(double) * n_dm);
+    if (!p->dm) { free_plan(p); return DEDISP_ENOMEM; }
+    memcpy(p->dm, dm, sizeof(double) * n_dm);
+
+    double* d_dm = nullptr;
+    auto fail = [&](int code) { if (d_dm) cudaFree(d_dm); free_plan(p); return code; };
+#define PLAN_TRY(expr)                                                                           \
+    do {                                                                                         \
+        cudaError_t e__ = (expr);                                                                \
+        if (e__ != cudaSuccess) {                                                                \
+            g_dedisp_last_cuda = (int)e__; (void)cudaGetLastError();                             \
+            return fail(e__ == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA);        \
+        }                                                                                        \
+    } while (0)
+    rc = dedisp_fused_init();
+    if (rc != DEDISP_OK) return fail(rc);
+    PLAN_TRY(cudaMalloc(&p->d_chirp, sizeof(float2) * (size_t)n_dm * n_chan * n_fft));
+    PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
+    if (n_dm > 1) PLAN_TRY(cudaMalloc(&p->d_spec, dedisp_fused_spec_bytes(n_fft)));
+    PLAN_TRY(cudaMalloc(&d_dm, sizeof(double) * n_dm));
+    PLAN_TRY(cudaMemcpy(d_dm, p->dm, sizeof(double) * n_dm, cudaMemcpyHostToDevice));
+    rc = dedisp_launch_chirp_table(p, d_dm, 0);
+    if (rc != DEDISP_OK) return fail(rc);
+    rc = dedisp_launch_twiddle_table(p->d_twiddle, n_fft, 0);
+    if (rc != DEDISP_OK) return fail(rc);
+    PLAN_TRY(cudaDeviceSynchronize());
+    cudaFree(d_dm);
+#undef PLAN_TRY
+    *out_plan = p;
+    return DEDISP_OK;
+}
+
+extern "C" int dedisp_get_info(dedisp_plan_t p, dedisp_info_t* info)
+{
+    if (!p || !info) return DEDISP_EINVAL;
+    info->n_chan = p->n_chan; info->n_dm = p->n_dm; info->n_fft = p->n_fft; info->n_int = p->n_int;
+    info->head = p->head; info->tail = p->tail; info->L = p->L;
+    info->chan_width_hz = p->bw_hz / p->n_chan;
+    info->max_smear_samples = p->max_smear_samples;
+    info->nfft_rule = p->nfft_rule;
+    return DEDISP_OK;
+}
+
+static long long n_blocks(const dedisp_plan_s* p, long long n_samp)
+{
+    if (n_samp < (long long)p->n_fft) return 0;
+    return (n_samp - p->head - p->tail) / p->L;
+}
+
+extern "C" long long dedisp_out_samples(dedisp_plan_t p, long long n_samp)
+{
+    if (!p) return DEDISP_EINVAL;
+    return n_blocks(p, n_samp) * (p->L / p->n_int);
+}
+
+extern "C" int dedisp_reserve(dedisp_plan_t p, long long n_samp)
+{
+    if (!p || n_samp <= 0) return DEDISP_EINVAL;
+    const long long stride = dedisp_xt_stride(n_samp);
+    if (stride <= p->xt_cap_samp) return DEDISP_OK;
+    DEDISP_CUDA_TRY(cudaDeviceSynchronize());
+    if (p->d_xt) { cudaFree(p->d_xt); p->d_xt = nullptr; p->xt_cap_samp = 0; }
+    DEDISP_CUDA_TRY(cudaMalloc(&p->d_xt, (size_t)stride * p->n_chan * 2));
+    p->xt_cap_samp = stride;
+    return DEDISP_OK;
+}
+
+extern "C" int dedisp_execute(dedisp_plan_t p, const int8_t* d_in, long long n_samp, float* d_out,
+                              long long out_stride, void* cuda_stream)
+{
+    if (!p || !d_in || n_samp <= 0) return DEDISP_EINVAL;
+    const long long nb = n_blocks(p, n_samp);
+    if (nb <= 0) return DEDISP_ESHORT;
+    if (!d_out) return DEDISP_EINVAL;
+    if (out_stride < nb * (p->L / p->n_int)) return DEDISP_EINVAL;
+    int rc = dedisp_reserve(p, n_samp);
+    if (rc != DEDISP_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long stride = p->xt_cap_samp;
+    // only the rows that complete blocks are needed: nb*L + head + tail
+    const long long used = nb * p->L + p->head + p->tail;
+    rc = dedisp_launch_corner_turn(d_in, used, p->n_chan, p->d_xt, stride, 0, st);
+    if (rc != DEDISP_OK) return rc;
+    return dedisp_launch_fused(p, p->d_xt, stride, nb, d_out, out_stride, 0, st);
+}
+
+extern "C" int dedisp_destroy(dedisp_plan_t p)
+{
+    if (!p) return DEDISP_EINVAL;
+    cudaDeviceSynchronize();
+    (void)cudaGetLastError();
+    free_plan(p);
+    return DEDISP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// test hooks
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" int dedisp_debug_chirp(dedisp_plan_t p, int d, int chan, float* h_chirp)
+{
+    if (!p || !h_chirp || d < 0 || d >= p->n_dm || chan < 0 || chan >= p->n_chan) return DEDISP_EINVAL;
+    DEDISP_CUDA_TRY(cudaMemcpy(h_chirp, p->d_chirp + ((size_t)d * p->n_chan + chan) * p->n_fft,
+                               sizeof(float2) * p->n_fft, cudaMemcpyDeviceToHost));
+    return DEDISP_OK;
+}
+
+static int debug_prepare(dedisp_plan_t p, const int8_t* d_in, long long n_samp, int chan, long long block,
+                         cudaStream_t st)
+{
+    if (!p || !d_in || chan < 0 || chan >= p->n_chan) return DEDISP_EINVAL;
+    const long long nb = n_blocks(p, n_samp);
+    if (nb <= 0) return DEDISP_ESHORT;
+    if (block < 0 || block >= nb) return DEDISP_EINVAL;
+    int rc = dedisp_reserve(p, n_samp);
+    if (rc != DEDISP_OK) return rc;
+    return dedisp_launch_corner_turn(d_in, nb * p->L + p->head + p->tail, p->n_chan, p->d_xt, p->xt_cap_samp, 0, st);
+}
+
+extern "C" int dedisp_debug_unpack(dedisp_plan_t p, const int8_t* d_in, long long n_samp, int chan, long long block,
+                                   float* d_block, void* cuda_stream)
+{
+    if (!d_block) return DEDISP_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = debug_prepare(p, d_in, n_samp, chan, block, st);
+    if (rc != DEDISP_OK) return rc;
+    return dedisp_launch_debug_unpack(p, p->d_xt, p->xt_cap_samp, chan, block, d_block, st);
+}
+
+extern "C" int dedisp_debug_voltage(dedisp_plan_t p, const int8_t* d_in, long long n_samp, int chan, long long block,
+                                    float* d_volt, void* cuda_stream)
+{
+    if (!d_volt) return DEDISP_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = debug_prepare(p, d_in, n_samp, chan, block, st);
+    if (rc != DEDISP_OK) return rc;
+    return dedisp_launch_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st);
+}

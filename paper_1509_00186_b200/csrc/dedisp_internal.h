@@ -1,0 +1,73 @@
+// Internal definitions shared by the translation units of libdedisp (product code; nothing here is used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "dedisp.h"
+
+// Dispersion constant of P:L117 ("4.148808 x 10^9" in MHz / us units) in Hz^2 s per pc cm^-3 (R8).
+#define DEDISP_D_HZ2_S 4.148808e15
+
+struct dedisp_stream_state;
+
+struct dedisp_plan_s {
+    // problem statement (observing frequency, bandwidth, DM) + channelisation and transform sizes
+    int n_chan, n_dm, n_fft, n_int;
+    double bw_hz, f_center_hz;
+    double* dm;  // host copy [n_dm]
+    unsigned flags;
+    // framing (R9)
+    int head, tail, L;
+    double max_smear_samples;
+    int nfft_rule;
+    int device;
+    // device tables owned by the plan
+    float2* d_chirp;    // [n_dm][n_chan][n_fft], taper * exp(+2 pi i psi) / n_fft
+    float2* d_twiddle;  // [n_fft], exp(-2 pi i m / n_fft)
+    // channel-major int8 scratch: [n_chan][xt_stride] (re,im) pairs, xt_stride samples per row
+    float2* d_spec;     // [resident CTAs][units per CTA][n_fft] forward-spectrum stash shared by the trial DMs (n_dm > 1)
+    int8_t* d_xt;
+    long long xt_cap_samp;  // samples per row the scratch can hold
+    dedisp_stream_state* stream;
+};
+
+extern thread_local int g_dedisp_last_cuda;
+
+#define DEDISP_CUDA_TRY(expr)                     \
+    do {                                          \
+        cudaError_t e__ = (expr);                 \
+        if (e__ != cudaSuccess) {                 \
+            g_dedisp_last_cuda = (int)e__;        \
+            (void)cudaGetLastError();             \
+            return e__ == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA; \
+        }                                         \
+    } while (0)
+
+// row stride (in samples) of the channel-major scratch for a call of n_samp samples: multiple of 64 samples
+// (= 128 B) so every block start b*L (L % 32 == 0) stays 64 B aligned for vector / bulk loads.
+static inline long long dedisp_xt_stride(long long n_samp) { return (n_samp + 63) / 64 * 64; }
+
+// kernels.cu / fused.cu launchers (all enqueue only)
+// corner turn: int8 [n_samp][n_chan][2] -> int8 [n_chan][xt_stride][2], rows t0_dst.. of the destination
+int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int8_t* d_xt, long long xt_stride,
+                              long long dst_t0, cudaStream_t st);
+// fused forward FFT -> chirp -> inverse FFT -> discard -> detect -> integrate over nb blocks of every channel.
+// out[d][c][out_col0 + b*L/n_int + j]
+int dedisp_launch_fused(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
+                        long long out_stride, long long out_col0, cudaStream_t st);
+int dedisp_launch_debug_unpack(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
+                               long long block, float* d_block, cudaStream_t st);
+int dedisp_launch_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
+                                long long block, float* d_volt, cudaStream_t st);
+int dedisp_fused_supported(int n_fft);
+size_t dedisp_fused_spec_bytes(int n_fft);  // valid after dedisp_fused_init()
+int dedisp_fused_init(void);  // sets the dynamic shared memory attributes once per process
+// plan-time table generation on the device (fp64 phase)
+int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaStream_t st);
+int dedisp_launch_twiddle_table(float2* d_tw, int n_fft, cudaStream_t st);
+// framing (R9) with the largest in-band smear (samples) reported as well
+int dedisp_framing_impl(int n_chan, double bw, double F, const double* dm, int n_dm, int n_fft, int n_int, int* head,
+                        int* tail, int* L, double* max_smear);
+// stream.cu
+void dedisp_stream_free(dedisp_plan_s* p);

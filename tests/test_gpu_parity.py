@@ -1,0 +1,199 @@
+"""GPU parity: the CUDA path (through the C ABI / ctypes binding) against the fp64 oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json:north_star's: per output block (the L/n_int outputs of one (dm, chan, block)) relative L2
+error <= 2e-5 and max |diff| <= 1e-3 * block RMS; the int8 unpack must be bit exact."""
+import os
+
+import numpy as np
+import pytest
+
+import datagen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+REL_L2_TOL = 2e-5     # north_star
+MAX_ABS_TOL = 1e-3    # x block RMS, north_star
+NT = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def dd():
+    import paper_1509_00186_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available()
+    return t
+
+
+def block_errors(got, ref, per):
+    """got/ref [n_dm][C][n_out] -> (worst rel-L2, worst max|d|/rms) over output blocks of `per` samples."""
+    g = np.asarray(got, dtype=np.float64).reshape(got.shape[0], got.shape[1], -1, per)
+    r = np.asarray(ref, dtype=np.float64).reshape(g.shape)
+    den = (r ** 2).sum(-1)
+    rel = np.sqrt(((g - r) ** 2).sum(-1) / np.where(den > 0, den, 1.0))
+    mx = np.abs(g - r).max(-1) / np.sqrt(np.where(den > 0, den / per, 1.0))
+    return float(rel.max()), float(mx.max())
+
+
+def assert_parity(got, ref, per):
+    assert got.shape == ref.shape
+    rel, mx = block_errors(got, ref, per)
+    assert rel <= REL_L2_TOL, f"block rel-L2 {rel:.3e} > {REL_L2_TOL}"
+    assert mx <= MAX_ABS_TOL, f"block max|d|/rms {mx:.3e} > {MAX_ABS_TOL}"
+    return rel, mx
+
+
+def make_plan(dd, w, **kw):
+    args = dict(n_chan=w.n_chan, bw_hz=w.bw_hz, f_center_hz=w.f_center_hz, dm=w.dm_trials, n_fft=w.n_fft,
+                n_int=w.n_int)
+    args.update(kw)
+    return dd.dedisp_plan(**args)
+
+
+def ocfg(w, **kw):
+    args = dict(n_chan=w.n_chan, bw_hz=w.bw_hz, f_center_hz=w.f_center_hz, dm=w.dm_trials, n_fft=w.n_fft,
+                n_int=w.n_int)
+    args.update(kw)
+    return oracle.OracleConfig(**args)
+
+
+def run_gpu(torch, plan, x):
+    out = plan.execute(torch.from_numpy(x).cuda())
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# framing + chirp table
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", datagen.WORKLOAD_ORDER)
+def test_plan_framing_matches_oracle(dd, name):
+    w = datagen.WORKLOADS[name]
+    with make_plan(dd, w) as plan:
+        assert (plan.head, plan.tail, plan.L) == oracle.framing(ocfg(w))
+        assert plan.info.chan_width_hz == w.bw_hz / w.n_chan
+
+
+@pytest.mark.parametrize("name,taper", [("tiny", "none"), ("gmrt32", "none"), ("lowfreq", "hann"),
+                                        ("wideband", "welch")])
+def test_chirp_table_matches_oracle_chirp(dd, name, taper):
+    """Table entries are fp32 roundings of taper*exp(2 pi i psi)/N with psi in fp64: error <= 1 ulp-ish of 1/N."""
+    w = datagen.WORKLOADS[name]
+    cfg = ocfg(w, taper=taper)
+    with make_plan(dd, w, taper=taper) as plan:
+        for d in sorted({0, plan.n_dm - 1}):
+            for c in (0, w.n_chan // 2, w.n_chan - 1):
+                h = plan.debug_chirp(d, c) * w.n_fft
+                ref = oracle.chirp(cfg, d, c)
+                assert np.abs(h - ref).max() <= 2.5e-7, (d, c, np.abs(h - ref).max())
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# unpack + corner turn: bit exact
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_chan,n_samp", [(64, 3000), (8, 2500), (5, 2100), (520, 2049)])
+def test_unpack_bit_exact_all_byte_values(dd, torch, n_chan, n_samp):
+    x = datagen.uniform_int8(n_samp, n_chan, seed=11)
+    x[:256, 0, 0] = np.arange(-128, 128, dtype=np.int8)   # every byte value at known places
+    x[:256, n_chan - 1, 1] = np.arange(-128, 128, dtype=np.int8)[::-1]
+    dm = (2.0,)
+    cfg = oracle.OracleConfig(n_chan, 16e6 * n_chan / 64, 325e6, dm, 1024, 4)
+    with dd.dedisp_plan(n_chan, cfg.bw_hz, 325e6, dm, 1024, 4) as plan:
+        xd = torch.from_numpy(x).cuda()
+        nb = plan.n_blocks(n_samp)
+        assert nb == oracle.n_blocks(cfg, n_samp) and nb >= 2
+        for c in sorted({0, 1, n_chan // 2, n_chan - 1}):
+            for b in (0, nb - 1):
+                got = plan.debug_unpack(xd, c, b).cpu().numpy()
+                ref = oracle.unpack_block(cfg, x, c, b)
+                assert np.array_equal(got.astype(np.float64), ref), (c, b)
+
+
+def test_dm_zero_is_integer_boxcar_power(dd, torch):
+    """P8: DM = 0 => H = 1 => out[j] is the integer sum of re^2+im^2 over rows head + j*n_int ...; pins unpack,
+    framing, block stitching, 1/N and the epilogue of the GPU path against a closed form (fp32 rounding only)."""
+    n_chan, n_samp, n_int = 24, 9000, 8
+    x = datagen.uniform_int8(n_samp, n_chan, seed=5)
+    with dd.dedisp_plan(n_chan, 6e6, 325e6, (0.0,), 2048, n_int) as plan:
+        got = run_gpu(torch, plan, x)[0]
+        head, L = plan.head, plan.L
+        n_out = plan.out_samples(n_samp)
+    p = (x.astype(np.int64) ** 2).sum(-1)                       # [t][c]
+    ref = p[head:head + n_out * n_int].reshape(n_out, n_int, n_chan).sum(1).T
+    assert got.shape == ref.shape
+    assert np.abs(got / ref - 1.0).max() < 5e-6
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# whole path vs oracle
+# ----------------------------------------------------------------------------------------------------------------
+def test_tiny_workload_full_parity(dd, torch):
+    w = datagen.WORKLOADS["tiny"]
+    x = datagen.generate(w)
+    ref = oracle.dedisp(ocfg(w), x, n_threads=NT)
+    with make_plan(dd, w) as plan:
+        got = run_gpu(torch, plan, x)
+        rel, mx = assert_parity(got, ref, plan.L // plan.n_int)
+    print(f"tiny: rel-L2 {rel:.2e} max/rms {mx:.2e}")
+
+
+@pytest.mark.parametrize("n_fft,n_int,dm,n_chan,taper", [
+    (1024, 16, (10.0,), 7, "none"),
+    (1024, 1, (-10.0,), 4, "hann"),
+    (2048, 8, (57.0,), 6, "none"),
+    (2048, 3, (20.0,), 5, "welch"),        # n_int not a power of two
+    (4096, 4, (71.0,), 4, "none"),
+    (4096, 64, (30.0, -30.0, 0.0), 3, "none"),
+    (8192, 32, (100.0,), 3, "none"),
+    (16384, 32, (150.0,), 3, "none"),
+    (16384, 64, (90.0, 100.0, 107.5), 2, "none"),
+    (16384, 96, (50.0,), 2, "hann"),       # n_int = 3 * 32
+])
+def test_small_cases_full_parity(dd, torch, n_fft, n_int, dm, n_chan, taper):
+    """Several blocks + a ragged tail per channel, every built transform size, multi-DM, both n_int paths."""
+    bw = 62.5e3 * n_chan
+    cfg = oracle.OracleConfig(n_chan, bw, 325e6 if n_fft < 16384 else 150e6, dm, n_fft, n_int, taper)
+    head, tail, L = oracle.framing(cfg)
+    n_samp = 3 * L + head + tail + 517        # 3 full blocks, ragged tail dropped
+    x = datagen.noise_only(n_samp, n_chan, seed=n_fft + n_int)
+    ref = oracle.dedisp(cfg, x, n_threads=NT)
+    with dd.dedisp_plan(n_chan, bw, cfg.f_center_hz, dm, n_fft, n_int, taper) as plan:
+        assert (plan.head, plan.tail, plan.L) == (head, tail, L)
+        got = run_gpu(torch, plan, x)
+        assert_parity(got, ref, L // n_int)
+
+
+def test_voltage_hook_matches_oracle_voltages(dd, torch):
+    w = datagen.WORKLOADS["gmrt32"].scaled(0.2)
+    chans = [0, 255, 511]
+    x = datagen.generate(w)
+    cfg = ocfg(w)
+    with make_plan(dd, w) as plan:
+        xd = torch.from_numpy(x).cuda()
+        nb = plan.n_blocks(x.shape[0])
+        for c in chans:
+            b = nb - 1
+            v = plan.debug_voltage(xd, c, b).cpu().numpy()
+            _, ref = oracle.dedisp_units(cfg, x, [c], [b], want_voltage=True)
+            got = v[..., 0] + 1j * v[..., 1]
+            err = np.linalg.norm(got - ref[0]) / np.linalg.norm(ref[0])
+            assert err < 2e-6, (c, err)
+
+
+def test_errors(dd, torch):
+    w = datagen.WORKLOADS["tiny"]
+    with pytest.raises(dd.DedispError):
+        make_plan(dd, w, n_fft=1000)
+    with pytest.raises(dd.DedispError):
+        make_plan(dd, w, dm=(100.0,))          # smear longer than the transform
+    with make_plan(dd, w) as plan:
+        short = torch.zeros((100, w.n_chan, 2), dtype=torch.int8, device="cuda")
+        with pytest.raises(dd.DedispError) as e:
+            plan.execute(short)
+        assert e.value.code == -4
+        assert plan.out_samples(100) == 0
