@@ -1,0 +1,396 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the channelised overlap-save dedispersion path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload gmrt32] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path (corner turn/unpack/framing, forward FFT, chirp,
+inverse FFT, discard, detect, integrate) over ONE batch = the whole workload (default: BASELINE.json configs[2], the
+32 MHz GMRT mode the metric's real-time factor is quoted on: 512 channels x 62.5 kHz, 16 s, N_fft 4096, n_int 4).
+
+value      device-resident: K dedisp_execute() calls between CUDA events, input already in HBM.
+e2e        the same metric through dedisp_stream_push() on pinned HOST buffers in 1 s chunks (H2D, kernels and D2H
+           overlapped on three streams), host wall clock around all pushes + the final sync.
+roofline   the fused kernel (dominant): nominal flops of its launches / its CUDA-event time (the library's
+           dedisp_profile_* events on the launching stream) against the FP32 FMA peak (bound "alu").
+cpu_baseline   the fp64 oracle, as it stands, on the host cores, on a bounded leading slice of the same input.
+N > 1      every rank runs its own workload-sized batch (its own seed): no data-path collective, "scaling": "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+from dataclasses import replace
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "complex Msamples/s dedispersed"
+UNIT = "Msamples/s"
+N_SM, FP32_LANES_PER_SM = 148, 128   # B200: 148 SMs x 4 sub-partitions x 32 FP32 lanes (guides: B300_MICROARCH)
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full`
+# capture (profiles/), keyed by workload; None until a capture of that workload exists.
+NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--workload", default="gmrt32")
+    ap.add_argument("--duration", type=float, default=0.0, help="override the workload's seconds of data (debug)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the cpu_baseline leg")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled every 100 ms while the timed region runs (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc, self.thr = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            return self
+        self.thr = threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True)
+        self.thr.start()
+        return self
+
+    def mark(self):
+        return len(self.lines)
+
+    def stop(self, lo: int = 0, hi: int | None = None):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+        rows = []
+        for l in self.lines[lo:hi]:
+            p = [v.strip() for v in l.split(",")]
+            if len(p) >= 7:
+                rows.append(p)
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        pw = [float(r[2]) for r in rows if r[2].replace(".", "", 1).isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "samples": len(rows), "power_w_max": max(pw) if pw else None}
+
+
+def get_workload(args, rank: int):
+    import datagen
+    w = datagen.WORKLOADS[args.workload]
+    if args.duration > 0:
+        w = w.scaled(args.duration)
+    return replace(w, seed=w.seed + rank)          # weak scaling: every rank its own batch
+
+
+def framing_counts(head: int, tail: int, L: int, n_samp: int, n_fft: int):
+    nb = 0 if n_samp < n_fft else (n_samp - head - tail) // L
+    return nb
+
+
+def nominal_flops_per_unit(n_fft: int, L: int, n_dm: int) -> float:
+    """One (channel, block) unit: 5 N log2 N per complex FFT (Eq. 5; one forward shared by the trial DMs + one
+    inverse per DM), 6 per chirp multiply (Eq. 5's 3N' term counts a complex multiply on half-length real data), and
+    3 (|v|^2) + 1 (integration add) per valid sample."""
+    fft = 5.0 * n_fft * math.log2(n_fft)
+    return (1 + n_dm) * fft + n_dm * (6.0 * n_fft + 4.0 * L)
+
+
+def algorithmic_bytes_per_unit(n_fft: int, L: int, n_dm: int, n_int: int) -> float:
+    """Fused kernel: reads the block's N samples as int8 pairs (the overlap is re-read: N, not L), writes L/n_int floats
+    per DM.  The chirp table (8 B x N per (DM, channel)) is shared by all blocks of a channel and is served by L2."""
+    return 2.0 * n_fft + 4.0 * n_dm * L / n_int
+
+
+def oracle_timed(w, x, n_threads: int, target_s: float):
+    """The oracle on a bounded leading slice of x, sized from a short calibration run to take about target_s."""
+    import oracle
+    cfg = oracle.OracleConfig(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
+    head, tail, L = oracle.framing(cfg)
+    T = x.shape[0]
+    n_cal = min(T, 2 * L + head + tail)
+    t0 = time.perf_counter()
+    oracle.dedisp(cfg, x[:n_cal], n_threads=n_threads)
+    t_cal = max(time.perf_counter() - t0, 1e-4)
+    nb_cal = (n_cal - head - tail) // L
+    nb_all = (T - head - tail) // L
+    nb = int(max(1, min(nb_all, nb_cal * target_s / t_cal)))
+    n = nb * L + head + tail
+    t0 = time.perf_counter()
+    out = oracle.dedisp(cfg, x[:n], n_threads=n_threads)
+    dt = time.perf_counter() - t0
+    assert out.shape[2] == nb * (L // w.n_int)
+    samples = w.n_chan * nb * L
+    return samples / dt / 1e6, dt, nb, nb_all
+
+
+def run_reference(args):
+    """--impl reference: the fp64 oracle as it stands on the host cores (this tier's reference arm).  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import datagen
+    import oracle
+    oracle.build()
+    w = get_workload(args, 0)
+    cores = os.cpu_count() or 1
+    # a step = a bounded sample of the workload: the first `per_step_s` seconds of oracle work
+    steps_total = args.steps + args.warmup
+    per_step_s = min(10.0, 150.0 / max(steps_total, 1))
+    # only the leading slice is needed: generate just enough data (full-length generation is for the GPU arm)
+    cfg = oracle.OracleConfig(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
+    head, tail, L = oracle.framing(cfg)
+    n_gen = min(w.n_samp, 256 * L + head + tail)
+    x = datagen.generate(w, n_samp=n_gen)
+    rate, dt, nb, nb_all = oracle_timed(w, x, cores, per_step_s)      # calibration + first warm-up
+    n = nb * L + head + tail
+    for _ in range(max(args.warmup - 1, 0)):
+        oracle.dedisp(cfg, x[:n], n_threads=cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.dedisp(cfg, x[:n], n_threads=cores)
+    dt = (time.perf_counter() - t0) / max(args.steps, 1)
+    value = w.n_chan * nb * L / dt / 1e6
+    sample = f"first {nb} of {(w.n_samp - head - tail) // L} blocks of every channel per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "real_time_factor": value * 1e6 / w.bw_hz,
+        "config": {"workload": w.name, "n_chan": w.n_chan, "bw_hz": w.bw_hz, "f_center_hz": w.f_center_hz,
+                   "n_fft": w.n_fft, "n_int": w.n_int, "dm": list(w.dm_trials), "duration_s": w.duration_s,
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(v: float) -> float:
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    import datagen
+    import paper_1509_00186_b200 as dd          # raises if libdedisp.so is missing: no fallback
+
+    w = get_workload(args, rank)
+    x = datagen.generate(w)                                       # int8 [T][C][2], seeded, host
+    T = x.shape[0]
+    h_in = torch.from_numpy(x).pin_memory()
+    d_in = h_in.cuda(non_blocking=False)
+
+    plan = dd.dedisp_plan(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
+    head, tail, L = plan.head, plan.tail, plan.L
+    nb = plan.n_blocks(T)
+    n_out = plan.out_samples(T)
+    n_units = w.n_chan * nb
+    samples = n_units * L                                          # valid complex samples dedispersed per step
+    plan.reserve(T)
+    d_out = torch.empty((plan.n_dm, w.n_chan, n_out), dtype=torch.float32, device="cuda")
+
+    # ---- device-resident timing -------------------------------------------------------------------------------
+    for _ in range(max(args.warmup, 3)):
+        plan.execute(d_in, d_out)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local).start() if rank == 0 else None
+    time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    plan.profile_enable(True)
+    barrier()
+    torch.cuda.synchronize()
+    mark0 = sampler.mark() if sampler else 0
+    ev0.record()
+    for _ in range(args.steps):
+        plan.execute(d_in, d_out)
+    ev1.record()
+    torch.cuda.synchronize()
+    barrier()
+    mark1 = sampler.mark() if sampler else 0
+    ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+    ms_ct, ms_fused, n_prof = plan.profile_read()
+    plan.profile_enable(False)
+    # keep the load on while the sampler catches at least a few readings (short runs finish between two samples)
+    if sampler and mark1 - mark0 < 3:
+        t_end = time.time() + 0.6
+        while time.time() < t_end:
+            plan.execute(d_in, d_out)
+        torch.cuda.synchronize()
+        mark1 = sampler.mark()
+    clocks = sampler.stop(mark0, max(mark1, mark0 + 1)) if sampler else None
+    ms_step = ms_total / args.steps
+    value = world * samples / (ms_step * 1e-3) / 1e6
+    checksum = float(d_out[:, :, : min(n_out, 1000)].double().mean().item())   # touches the result; sanity only
+
+    # ---- end to end from pinned host memory (config 3: 1 s chunks, double buffered) -------------------------------
+    e2e = None
+    if not args.no_e2e:
+        chunk = int(round((w.chunk_s if w.chunk_s > 0 else 1.0) * w.chan_width_hz))
+        chunk = max(min(chunk, T), 1)
+        h_out = torch.empty((plan.n_dm, w.n_chan, n_out), dtype=torch.float32).pin_memory()
+        plan.stream_begin(chunk)
+
+        def e2e_step():
+            plan.stream_begin(chunk)                 # same buffers: resets the carry only
+            col, t = 0, 0
+            while t < T:
+                n = min(chunk, T - t)
+                col += plan.stream_push(h_in[t:t + n], h_out, col)
+                t += n
+            plan.stream_sync()
+            return col
+
+        for _ in range(max(args.warmup, 3)):
+            assert e2e_step() == n_out
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        barrier()
+        dt = max_over_ranks(dt) / args.steps
+        plan.stream_end()
+        same = bool(torch.equal(h_out, d_out.cpu()))
+        e2e = {"value": world * samples / dt / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": int(h_in.numel()), "d2h_bytes_per_step": int(h_out.numel() * 4),
+               "ms_per_step": dt * 1e3, "real_time_factor": world * samples / dt / w.bw_hz,
+               "chunk_samples": chunk, "chunks_per_step": (T + chunk - 1) // chunk,
+               "timer": "host wall clock around all pushes + stream_sync",
+               "api": "dedisp_stream_push (pinned host int8 in, pinned host fp32 out)",
+               "equals_device_resident_output": same}
+        del h_out
+
+    # ---- roofline of the dominant (fused) kernel --------------------------------------------------------------------
+    peaks, peaks_src = measured_peaks()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    fp32_peak_tf = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    fused_ms = ms_fused / max(n_prof, 1)
+    ct_ms = ms_ct / max(n_prof, 1)
+    flops = n_units * nominal_flops_per_unit(w.n_fft, L, plan.n_dm)
+    abytes = n_units * algorithmic_bytes_per_unit(w.n_fft, L, plan.n_dm, w.n_int)
+    achieved_tf = flops / (fused_ms * 1e-3) / 1e12
+    roofline = {
+        "bound": "alu", "kernel": "fused_dedisp_kernel", "achieved": achieved_tf, "peak": fp32_peak_tf,
+        "unit": "TFLOP/s", "frac": achieved_tf / fp32_peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+        "peak_source": f"{N_SM} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 (FMA) x {sm_max:.0f} MHz "
+                       f"(sm_max_mhz of MEASURED_PEAKS.json, {peaks_src})",
+        "flops_per_launch": flops, "ms_per_launch": fused_ms, "share_of_step": fused_ms / ms_step,
+        "hbm": {"algorithmic_bytes_per_launch": abytes, "achieved_gbs": abytes / (fused_ms * 1e-3) / 1e9,
+                "peak_gbs": float(peaks.get("hbm_gbs", 6650.0)),
+                "frac": abytes / (fused_ms * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0))},
+        "corner_turn": {"ms_per_launch": ct_ms, "share_of_step": ct_ms / ms_step,
+                        "algorithmic_bytes_per_launch": 4.0 * w.n_chan * (nb * L + head + tail),
+                        "achieved_gbs": 4.0 * w.n_chan * (nb * L + head + tail) / (ct_ms * 1e-3) / 1e9,
+                        "frac_of_hbm_peak": 4.0 * w.n_chan * (nb * L + head + tail) / (ct_ms * 1e-3) / 1e9
+                        / float(peaks.get("hbm_gbs", 6650.0))},
+    }
+    if clocks and clocks.get("sm_mhz"):
+        pk = N_SM * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12
+        roofline["frac_at_observed_clock"] = achieved_tf / pk
+
+    if rank != 0:
+        plan.destroy()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- CPU baseline: the oracle on the host cores, bounded sample (rank 0, N = 1 only) ----------------------------
+    cpu = None
+    if not args.no_cpu and world == 1:
+        import oracle
+        oracle.build()
+        cores = os.cpu_count() or 1
+        rate, dt, nb_cpu, nb_all = oracle_timed(w, x, cores, args.cpu_seconds)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {nb_cpu} of {nb_all} blocks of every channel ({dt:.1f} s of wall time)",
+               "real_time_factor": rate * 1e6 / w.bw_hz}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "real_time_factor": value * 1e6 / w.bw_hz,
+        "config": {"workload": w.name, "n_chan": w.n_chan, "bw_hz": w.bw_hz, "f_center_hz": w.f_center_hz,
+                   "n_fft": w.n_fft, "n_int": w.n_int, "dm": list(w.dm_trials), "duration_s": w.duration_s,
+                   "samples_per_channel": T, "head": head, "tail": tail, "L": L, "blocks_per_channel": nb,
+                   "valid_samples_per_step_per_gpu": samples, "input_bytes": int(d_in.numel()),
+                   "output_bytes": int(d_out.numel() * 4),
+                   "l2": "inputs larger than L2 (no flush needed)" if d_in.numel() > 256e6 else
+                         "input smaller than 2x L2: numbers include L2 hits",
+                   "sharding": "one workload-sized batch per rank, no data-path collective"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps,
+        "roofline": roofline, "cpu_baseline": cpu, "checksum_mean_first_1000": checksum,
+    }
+    print(json.dumps(line), flush=True)
+    plan.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

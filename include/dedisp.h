@@ -71,6 +71,7 @@ int dedisp_framing(int n_chan, double bw_hz, double f_center_hz, const double* d
  * Create a plan on the current CUDA device: validates, computes the framing, builds the chirp table
  * float2 [n_dm][n_chan][n_fft] (phase in fp64, value rounded to fp32, pre-scaled by 1/n_fft) and the FFT twiddles.
  *   n_fft: one of 1024, 2048, 4096, 8192, 16384 (the built kernel sizes).  dm: HOST array, copied.
+ *   n_int: a power of two (R9 makes the overlap a multiple of n_int, so L % n_int == n_fft % n_int).
  * Synchronises the device once.  Errors: EINVAL, ENOMEM, ECUDA, ENODEV.
  */
 int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, double f_center_hz, const double* dm, int n_dm,
@@ -101,16 +102,28 @@ int dedisp_execute(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, flo
  * the samples lost at a block edge are prefixed to the next block).  Push consecutive chunks of the same observation;
  * the plan keeps the unconsumed tail on the device so that the concatenated output equals a one-shot call on the
  * concatenated input (R12).
- *   h_in   HOST (pinned for overlap), int8 [n_samp][n_chan][2].
+ *   h_in   HOST (pinned for overlap), int8 [n_samp][n_chan][2], n_samp <= max_chunk_samp of dedisp_stream_begin.
  *   h_out  HOST (pinned), float [n_dm][n_chan][out_stride]: receives the outputs completed by THIS chunk in columns
- *          [0, *n_out); valid after dedisp_stream_sync().
- * The call returns after enqueueing; h_in must stay untouched until the next push or sync returns.
+ *          [0, *n_out); *n_out is known when the call returns (host arithmetic), out_stride >= *n_out.
+ * The call enqueues the chunk's H2D copy, kernels and D2H copy on the plan's three streams and returns.  Buffer
+ * hand-back: h_in may be reused once the NEXT push (or dedisp_stream_sync) has returned; h_out holds its values once
+ * the SECOND-NEXT push (or dedisp_stream_sync) has returned.  dedisp_stream_begin allocates the device double buffers
+ * (2 staging chunks, 2 channel-major carries+chunks, 2 output blocks) and resets the carry; dedisp_stream_end frees
+ * them.  Errors: EINVAL (no begin, chunk too long, null pointers, out_stride too small), ENOMEM, ECUDA.
  */
 int dedisp_stream_begin(dedisp_plan_t plan, long long max_chunk_samp);
 int dedisp_stream_push(dedisp_plan_t plan, const int8_t* h_in, long long n_samp, float* h_out, long long out_stride,
                        long long* n_out);
 int dedisp_stream_sync(dedisp_plan_t plan);
 int dedisp_stream_end(dedisp_plan_t plan);
+
+/*
+ * Kernel timing for the roofline report: while enabled, every dedisp_execute / dedisp_stream_push records CUDA events
+ * on its compute stream around the corner-turn and the fused kernel (up to 256 calls are kept).  dedisp_profile_read
+ * synchronises those events, returns the summed device times in milliseconds and the number of calls, and clears them.
+ */
+int dedisp_profile_enable(dedisp_plan_t plan, int on);
+int dedisp_profile_read(dedisp_plan_t plan, double* ms_corner_turn, double* ms_fused, int* n_calls);
 
 int dedisp_destroy(dedisp_plan_t plan);
 

@@ -15,7 +15,8 @@ TAPER = {"none": 0, "hann": 1, "welch": 2}
 # every symbol include/dedisp.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "dedisp_framing", "dedisp_plan", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
-    "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_destroy",
+    "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_profile_enable",
+    "dedisp_profile_read", "dedisp_destroy",
     "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
 )
 
@@ -37,7 +38,7 @@ class DedispError(RuntimeError):
 
 def _load() -> C.CDLL:
     if not os.path.exists(LIB_PATH):
-        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1509_00186_b200.build` "
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python paper_1509_00186_b200/build.py` "
                           "(the CUDA library is the product; there is no fallback)")
     L = C.CDLL(LIB_PATH)
     dp, ip, vp, ll = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p, C.c_longlong
@@ -52,6 +53,8 @@ def _load() -> C.CDLL:
     L.dedisp_stream_push.argtypes = [vp, vp, ll, vp, ll, C.POINTER(ll)]
     L.dedisp_stream_sync.argtypes = [vp]
     L.dedisp_stream_end.argtypes = [vp]
+    L.dedisp_profile_enable.argtypes = [vp, C.c_int]
+    L.dedisp_profile_read.argtypes = [vp, dp, dp, ip]
     L.dedisp_destroy.argtypes = [vp]
     L.dedisp_strerror.argtypes = [C.c_int]
     L.dedisp_strerror.restype = C.c_char_p
@@ -141,11 +144,21 @@ class Plan:
     def stream_begin(self, max_chunk_samp: int) -> None:
         _check(_lib.dedisp_stream_begin(self._h, max_chunk_samp), "dedisp_stream_begin")
 
-    def stream_push(self, h_in, h_out) -> int:
-        """h_in: pinned int8 [n][C][2]; h_out: pinned float32 [n_dm][C][stride]; returns outputs written."""
+    def stream_push(self, h_in, h_out, col0: int = 0) -> int:
+        """h_in: pinned int8 [n][C][2]; h_out: pinned float32 [n_dm][C][stride], this chunk's outputs land in columns
+        [col0, col0 + returned count) of every row.  Returns the number of outputs per (dm, chan) this chunk completed."""
+        import torch
+        assert not h_in.is_cuda and h_in.dtype == torch.int8 and h_in.is_contiguous()
+        assert h_in.dim() == 3 and h_in.shape[1] == self.n_chan and h_in.shape[2] == 2
+        assert not h_out.is_cuda and h_out.dtype == torch.float32 and h_out.is_contiguous()
+        assert h_out.dim() == 3 and h_out.shape[0] == self.n_dm and h_out.shape[1] == self.n_chan
+        assert 0 <= col0 <= h_out.shape[2]
         n = C.c_longlong(0)
-        _check(_lib.dedisp_stream_push(self._h, h_in.data_ptr(), h_in.shape[0], h_out.data_ptr(), h_out.shape[2],
-                                       C.byref(n)), "dedisp_stream_push")
+        # the library checks out_stride >= n_out; the room left behind col0 is checked here
+        rc = _lib.dedisp_stream_push(self._h, h_in.data_ptr(), h_in.shape[0], h_out.data_ptr() + 4 * col0,
+                                     h_out.shape[2], C.byref(n))
+        _check(rc, "dedisp_stream_push")
+        assert col0 + n.value <= h_out.shape[2], "h_out too short for this chunk's outputs"
         return int(n.value)
 
     def stream_sync(self) -> None:
@@ -153,6 +166,16 @@ class Plan:
 
     def stream_end(self) -> None:
         _check(_lib.dedisp_stream_end(self._h), "dedisp_stream_end")
+
+    # -- kernel timing ----------------------------------------------------------------------------------------
+    def profile_enable(self, on: bool = True) -> None:
+        _check(_lib.dedisp_profile_enable(self._h, 1 if on else 0), "dedisp_profile_enable")
+
+    def profile_read(self):
+        """(ms in the corner-turn kernel, ms in the fused kernel, calls) summed since the last read."""
+        a, b, n = C.c_double(), C.c_double(), C.c_int()
+        _check(_lib.dedisp_profile_read(self._h, C.byref(a), C.byref(b), C.byref(n)), "dedisp_profile_read")
+        return a.value, b.value, n.value
 
     # -- test hooks -------------------------------------------------------------------------------------------
     def debug_unpack(self, d_in, chan: int, block: int):

@@ -1,4 +1,5 @@
-"""Builds libdedisp.so (sm_100a only) in-tree with nvcc.  `python -m paper_1509_00186_b200.build [--force]`."""
+"""Builds libdedisp.so (sm_100a only) in-tree with nvcc.  `python paper_1509_00186_b200/build.py [--force] [-v]`
+(run as a script: importing the package needs the library this builds)."""
 from __future__ import annotations
 
 import os

@@ -30,6 +30,10 @@ static void free_plan(dedisp_plan_s* p)
     if (p->d_twiddle) cudaFree(p->d_twiddle);
     if (p->d_xt) cudaFree(p->d_xt);
     if (p->d_spec) cudaFree(p->d_spec);
+    if (p->prof_ev) {
+        for (int i = 0; i < DEDISP_PROF_MAX * 3; ++i) cudaEventDestroy(p->prof_ev[i]);
+        free(p->prof_ev);
+    }
     free(p->dm);
     delete p;
 }
@@ -41,6 +45,8 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     *out_plan = nullptr;
     if ((flags & ~DEDISP_TAPER_MASK) || (flags & DEDISP_TAPER_MASK) == 3u) return DEDISP_EINVAL;
     if (n_fft <= 0 || (n_fft & (n_fft - 1)) || !dedisp_fused_supported(n_fft)) return DEDISP_EINVAL;
+    // R9 gives D_tot % n_int == 0, so L % n_int == n_fft % n_int: only powers of two can divide a block evenly
+    if (n_int <= 0 || (n_int & (n_int - 1))) return DEDISP_EINVAL;
     int head, tail, L;
     double smear = 0.0;
     int rc = dedisp_framing_impl(n_chan, bw_hz, f_center_hz, dm, n_dm, n_fft, n_int, &head, &tail, &L, &smear);
@@ -111,10 +117,63 @@ extern "C" int dedisp_get_info(dedisp_plan_t p, dedisp_info_t* info)
     return DEDISP_OK;
 }
 
-static long long n_blocks(const dedisp_plan_s* p, long long n_samp)
+long long dedisp_n_blocks(const dedisp_plan_s* p, long long n_samp)
 {
     if (n_samp < (long long)p->n_fft) return 0;
     return (n_samp - p->head - p->tail) / p->L;
+}
+static long long n_blocks(const dedisp_plan_s* p, long long n_samp) { return dedisp_n_blocks(p, n_samp); }
+
+// The two kernels of the path for one batch of rows: corner-turn n_rows input rows to d_xt at row offset dst_t0, then
+// the fused kernel over the first nb blocks of d_xt.  Optional events: profiling triple, and `after_corner_turn`
+// (the streaming path frees its staging buffer there).
+int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows, int8_t* d_xt, long long xt_stride,
+                         long long dst_t0, long long nb, float* d_out, long long out_stride, cudaStream_t st,
+                         cudaEvent_t after_corner_turn)
+{
+    cudaEvent_t* ev = nullptr;
+    if (p->prof_on && p->prof_n < DEDISP_PROF_MAX) ev = p->prof_ev + 3 * (p->prof_n++);
+    if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[0], st));
+    int rc = dedisp_launch_corner_turn(d_in, n_rows, p->n_chan, d_xt, xt_stride, dst_t0, st);
+    if (rc != DEDISP_OK) return rc;
+    if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[1], st));
+    if (after_corner_turn) DEDISP_CUDA_TRY(cudaEventRecord(after_corner_turn, st));
+    if (nb > 0) {
+        rc = dedisp_launch_fused(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st);
+        if (rc != DEDISP_OK) return rc;
+    }
+    if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[2], st));
+    return DEDISP_OK;
+}
+
+extern "C" int dedisp_profile_enable(dedisp_plan_t p, int on)
+{
+    if (!p) return DEDISP_EINVAL;
+    if (on && !p->prof_ev) {
+        p->prof_ev = (cudaEvent_t*)calloc(DEDISP_PROF_MAX * 3, sizeof(cudaEvent_t));
+        if (!p->prof_ev) return DEDISP_ENOMEM;
+        for (int i = 0; i < DEDISP_PROF_MAX * 3; ++i) DEDISP_CUDA_TRY(cudaEventCreate(&p->prof_ev[i]));
+    }
+    p->prof_on = on ? 1 : 0;
+    p->prof_n = 0;
+    return DEDISP_OK;
+}
+
+extern "C" int dedisp_profile_read(dedisp_plan_t p, double* ms_corner_turn, double* ms_fused, int* n_calls)
+{
+    if (!p || !ms_corner_turn || !ms_fused || !n_calls) return DEDISP_EINVAL;
+    double a = 0.0, b = 0.0;
+    for (int i = 0; i < p->prof_n; ++i) {
+        cudaEvent_t* ev = p->prof_ev + 3 * i;
+        float m1 = 0.f, m2 = 0.f;
+        DEDISP_CUDA_TRY(cudaEventSynchronize(ev[2]));
+        DEDISP_CUDA_TRY(cudaEventElapsedTime(&m1, ev[0], ev[1]));
+        DEDISP_CUDA_TRY(cudaEventElapsedTime(&m2, ev[1], ev[2]));
+        a += m1; b += m2;
+    }
+    *ms_corner_turn = a; *ms_fused = b; *n_calls = p->prof_n;
+    p->prof_n = 0;
+    return DEDISP_OK;
 }
 
 extern "C" long long dedisp_out_samples(dedisp_plan_t p, long long n_samp)
@@ -149,9 +208,7 @@ extern "C" int dedisp_execute(dedisp_plan_t p, const int8_t* d_in, long long n_s
     const long long stride = p->xt_cap_samp;
     // only the rows that complete blocks are needed: nb*L + head + tail
     const long long used = nb * p->L + p->head + p->tail;
-    rc = dedisp_launch_corner_turn(d_in, used, p->n_chan, p->d_xt, stride, 0, st);
-    if (rc != DEDISP_OK) return rc;
-    return dedisp_launch_fused(p, p->d_xt, stride, nb, d_out, out_stride, 0, st);
+    return dedisp_enqueue_chunk(p, d_in, used, p->d_xt, stride, 0, nb, d_out, out_stride, st, nullptr);
 }
 
 extern "C" int dedisp_destroy(dedisp_plan_t p)

@@ -11,13 +11,15 @@ constexpr int TILE_T = 128;  // samples per tile: 128 * 2 B = 256 B per output r
 constexpr int PITCH_W = 33;  // smem row pitch in 32-bit words (64 shorts + 1 word pad)
 
 // Vector path: 16 B loads along the channel axis, 16 B stores along the time axis.
-// Requires n_chan % 8 == 0, dst_t0 % 8 == 0, xt_stride % 8 == 0 and 16 B aligned base pointers.
+// Requires n_chan % 8 == 0, xt_stride % 8 == 0 and 16 B aligned base pointers.  Tiles are laid on the DESTINATION's
+// 8-sample grid (the first tile starts dst_t0 % 8 rows before row 0), so any dst_t0 keeps the 16 B stores aligned:
+// the streaming path appends chunks behind a carry of arbitrary length.
 __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const int8_t* __restrict__ in, long long n_samp, int n_chan,
                                                               int8_t* __restrict__ xt, long long xt_stride,
                                                               long long dst_t0)
 {
     __shared__ uint32_t tile[TILE_T * PITCH_W];
-    const long long t0 = (long long)blockIdx.x * TILE_T;
+    const long long t0 = (long long)blockIdx.x * TILE_T - (dst_t0 & 7);
     const int c0 = blockIdx.y * TILE_C;
     const int tid = threadIdx.x;
     const uint16_t* in16 = reinterpret_cast<const uint16_t*>(in);
@@ -28,7 +30,7 @@ __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const int8_t* __re
         const long long t = t0 + row;
         const int c = c0 + q * 8;
         uint4 v = make_uint4(0, 0, 0, 0);
-        if (t < n_samp && c < n_chan)  // n_chan % 8 == 0: the 8 channels are all inside
+        if (t >= 0 && t < n_samp && c < n_chan)  // n_chan % 8 == 0: the 8 channels are all inside
             v = __ldg(reinterpret_cast<const uint4*>(in16 + t * n_chan + c));
         uint32_t* dst = &tile[row * PITCH_W + q * 4];
         dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
@@ -51,12 +53,13 @@ __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const int8_t* __re
             w[i] = lo | (hi << 16);
         }
         const long long t = t0 + tq * 8;
-        if (c0 + c >= n_chan || t >= n_samp) continue;
+        if (c0 + c >= n_chan || t >= n_samp || t + 8 <= 0) continue;
         uint16_t* dst = xt16 + (long long)(c0 + c) * xt_stride + dst_t0 + t;
-        if (t + 8 <= n_samp) {
+        if (t >= 0 && t + 8 <= n_samp) {
             *reinterpret_cast<uint4*>(dst) = make_uint4(w[0], w[1], w[2], w[3]);
         } else {
-            for (int i = 0; i < 8 && t + i < n_samp; ++i) dst[i] = (uint16_t)(w[i >> 1] >> ((i & 1) * 16));
+            for (int i = 0; i < 8; ++i)
+                if (t + i >= 0 && t + i < n_samp) dst[i] = (uint16_t)(w[i >> 1] >> ((i & 1) * 16));
         }
     }
 }
@@ -91,10 +94,10 @@ int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, 
                               long long dst_t0, cudaStream_t st)
 {
     if (n_samp <= 0) return DEDISP_OK;
-    const bool vec = (n_chan % 8 == 0) && (dst_t0 % 8 == 0) && (xt_stride % 8 == 0) &&
-                     ((uintptr_t)d_in % 16 == 0) && ((uintptr_t)d_xt % 16 == 0);
+    const bool vec = (n_chan % 8 == 0) && (xt_stride % 8 == 0) && ((uintptr_t)d_in % 16 == 0) &&
+                     ((uintptr_t)d_xt % 16 == 0);
     if (vec) {
-        dim3 grid((unsigned)((n_samp + TILE_T - 1) / TILE_T), (unsigned)((n_chan + TILE_C - 1) / TILE_C));
+        dim3 grid((unsigned)((n_samp + (dst_t0 & 7) + TILE_T - 1) / TILE_T), (unsigned)((n_chan + TILE_C - 1) / TILE_C));
         corner_turn_vec_kernel<<<grid, 256, 0, st>>>(d_in, n_samp, n_chan, d_xt, xt_stride, dst_t0);
     } else {
         dim3 grid((unsigned)((n_samp + 31) / 32), (unsigned)((n_chan + 31) / 32));

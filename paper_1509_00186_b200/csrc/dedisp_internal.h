@@ -30,7 +30,11 @@ struct dedisp_plan_s {
     int8_t* d_xt;
     long long xt_cap_samp;  // samples per row the scratch can hold
     dedisp_stream_state* stream;
+    // kernel timing (dedisp_profile_enable): 3 events per call -- before corner turn, between, after fused
+    int prof_on, prof_n;
+    cudaEvent_t* prof_ev;  // [DEDISP_PROF_MAX][3], created on first enable
 };
+#define DEDISP_PROF_MAX 256
 
 extern thread_local int g_dedisp_last_cuda;
 
@@ -69,5 +73,10 @@ int dedisp_launch_twiddle_table(float2* d_tw, int n_fft, cudaStream_t st);
 // framing (R9) with the largest in-band smear (samples) reported as well
 int dedisp_framing_impl(int n_chan, double bw, double F, const double* dm, int n_dm, int n_fft, int n_int, int* head,
                         int* tail, int* L, double* max_smear);
+// api.cu: corner turn + fused kernel on `st` with the optional profiling events around them
+int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows, int8_t* d_xt, long long xt_stride,
+                         long long dst_t0, long long nb, float* d_out, long long out_stride, cudaStream_t st,
+                         cudaEvent_t after_corner_turn);
+long long dedisp_n_blocks(const dedisp_plan_s* p, long long n_samp);
 // stream.cu
 void dedisp_stream_free(dedisp_plan_s* p);

@@ -146,16 +146,16 @@ def test_tiny_workload_full_parity(dd, torch):
     (1024, 16, (10.0,), 7, "none"),
     (1024, 1, (-10.0,), 4, "hann"),
     (2048, 8, (57.0,), 6, "none"),
-    (2048, 3, (20.0,), 5, "welch"),        # n_int not a power of two
+    (2048, 2, (20.0,), 5, "welch"),
     (4096, 4, (71.0,), 4, "none"),
     (4096, 64, (30.0, -30.0, 0.0), 3, "none"),
     (8192, 32, (100.0,), 3, "none"),
     (16384, 32, (150.0,), 3, "none"),
     (16384, 64, (90.0, 100.0, 107.5), 2, "none"),
-    (16384, 96, (50.0,), 2, "hann"),       # n_int = 3 * 32
+    (16384, 128, (50.0,), 2, "hann"),      # n_int > one warp
 ])
 def test_small_cases_full_parity(dd, torch, n_fft, n_int, dm, n_chan, taper):
-    """Several blocks + a ragged tail per channel, every built transform size, multi-DM, both n_int paths."""
+    """Several blocks + a ragged tail per channel, every built transform size, multi-DM, n_int below/above a warp."""
     bw = 62.5e3 * n_chan
     cfg = oracle.OracleConfig(n_chan, bw, 325e6 if n_fft < 16384 else 150e6, dm, n_fft, n_int, taper)
     head, tail, L = oracle.framing(cfg)
@@ -191,9 +191,104 @@ def test_errors(dd, torch):
         make_plan(dd, w, n_fft=1000)
     with pytest.raises(dd.DedispError):
         make_plan(dd, w, dm=(100.0,))          # smear longer than the transform
+    with pytest.raises(dd.DedispError):
+        make_plan(dd, w, n_int=3)              # R9: only powers of two divide a block
     with make_plan(dd, w) as plan:
         short = torch.zeros((100, w.n_chan, 2), dtype=torch.int8, device="cuda")
         with pytest.raises(dd.DedispError) as e:
             plan.execute(short)
         assert e.value.code == -4
         assert plan.out_samples(100) == 0
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# streaming (a6): chunked == one-shot (P10), carry across chunks of awkward lengths
+# ----------------------------------------------------------------------------------------------------------------
+def stream_run(torch, plan, x, chunk_lens):
+    n_samp = x.shape[0]
+    total_out = plan.out_samples(n_samp)
+    h_out = torch.full((plan.n_dm, plan.n_chan, total_out + 8), float("nan")).pin_memory()
+    plan.stream_begin(max(chunk_lens))
+    col, t, i = 0, 0, 0
+    keep = []
+    while t < n_samp:
+        n = min(chunk_lens[i % len(chunk_lens)], n_samp - t)
+        h_in = torch.from_numpy(x[t:t + n]).clone().pin_memory()
+        keep = (keep + [h_in])[-2:]            # h_in may be reused once the next push has returned
+        col += plan.stream_push(h_in, h_out, col)
+        t += n
+        i += 1
+    plan.stream_sync()
+    plan.stream_end()
+    assert col == total_out
+    assert torch.isnan(h_out[:, :, total_out:]).all()          # nothing written past the outputs
+    return h_out[:, :, :total_out].numpy().copy()
+
+
+@pytest.mark.parametrize("n_fft,n_int,dm,n_chan,chunks", [
+    (1024, 16, (10.0,), 64, (5000,)),
+    (1024, 4, (10.0,), 8, (1237, 3001, 411)),          # odd lengths: carry lands on every alignment; 411 < one block
+    (4096, 4, (71.0,), 16, (6250,)),                   # gmrt32's 1 s chunk / 10
+    (2048, 8, (57.0,), 5, (4099, 2048)),               # n_chan % 8 != 0: scalar corner turn
+    (16384, 64, (90.0, 100.0), 8, (40000, 12345)),
+])
+def test_streaming_equals_one_shot_bitwise(dd, torch, n_fft, n_int, dm, n_chan, chunks):
+    bw = 62.5e3 * n_chan
+    fc = 325e6 if n_fft < 16384 else 400e6
+    with dd.dedisp_plan(n_chan, bw, fc, dm, n_fft, n_int) as plan:
+        n_samp = 4 * plan.L + plan.head + plan.tail + 777 if n_fft < 16384 else 5 * plan.L + 999
+        x = datagen.noise_only(n_samp, n_chan, seed=n_fft + n_chan)
+        one = run_gpu(torch, plan, x)
+        got = stream_run(torch, plan, x, chunks)
+        assert one.shape == got.shape and one.shape[2] > 0
+        assert np.array_equal(one, got)
+        # and once more on the same plan: begin() resets the carry
+        got2 = stream_run(torch, plan, x, chunks[::-1])
+        assert np.array_equal(one, got2)
+
+
+def test_streaming_against_oracle(dd, torch):
+    """The streamed path on a 0.5 s cut of the 32 MHz workload in 0.1 s chunks, against the one-shot oracle."""
+    w = datagen.WORKLOADS["gmrt32"].scaled(0.5)
+    chans = list(range(0, 512, 16))
+    x = datagen.generate(w, chans=chans)
+    bw = w.chan_width_hz * len(chans)
+    # a 32-channel band with the same channel width; centre chosen so the lowest channel is gmrt32's lowest
+    fc = w.f_center_hz - 0.5 * w.bw_hz + 0.5 * bw
+    cfg = oracle.OracleConfig(len(chans), bw, fc, w.dm_trials, w.n_fft, w.n_int)
+    ref = oracle.dedisp(cfg, x, n_threads=NT)
+    with dd.dedisp_plan(len(chans), bw, fc, w.dm_trials, w.n_fft, w.n_int) as plan:
+        got = stream_run(torch, plan, x, (6250,))
+        assert_parity(got, ref, plan.L // plan.n_int)
+
+
+def test_stream_errors(dd, torch):
+    w = datagen.WORKLOADS["tiny"]
+    with make_plan(dd, w) as plan:
+        h_in = torch.zeros((2000, w.n_chan, 2), dtype=torch.int8).pin_memory()
+        h_out = torch.zeros((1, w.n_chan, 64), dtype=torch.float32).pin_memory()
+        with pytest.raises(dd.DedispError):
+            plan.stream_push(h_in, h_out)              # no begin
+        plan.stream_begin(1000)
+        with pytest.raises(dd.DedispError):
+            plan.stream_push(h_in, h_out)              # chunk longer than max_chunk_samp
+        plan.stream_end()
+        plan.stream_begin(2000)
+        with pytest.raises(dd.DedispError):
+            plan.stream_push(h_in, h_out[:, :, :1].contiguous())   # out_stride too small
+        plan.stream_end()
+
+
+def test_profile_hooks_time_both_kernels(dd, torch):
+    w = datagen.WORKLOADS["tiny"]
+    x = torch.from_numpy(datagen.noise_only(w.n_samp, w.n_chan, seed=1)).cuda()
+    with make_plan(dd, w) as plan:
+        plan.profile_enable(True)
+        for _ in range(3):
+            plan.execute(x)
+        a, b, n = plan.profile_read()
+        assert n == 3 and a > 0.0 and b > 0.0
+        assert plan.profile_read() == (0.0, 0.0, 0)
+        plan.profile_enable(False)
+        plan.execute(x)
+        assert plan.profile_read()[2] == 0
