@@ -109,6 +109,22 @@ class ClockSampler:
                 "samples": len(rows), "power_w_max": max(pw) if pw else None}
 
 
+def reduce_max_over_ranks(v: float, world: int, device: str) -> float:
+    """Timing rule: a multi-rank time is the MAX over ranks (the only collective bench.py issues besides barriers)."""
+    if world == 1:
+        return v
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([v], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(samples_per_rank: int, world: int, seconds_per_step: float) -> float:
+    """Msamples/s over all ranks: every rank dedisperses its own batch of `samples_per_rank` valid samples per step."""
+    return world * samples_per_rank / seconds_per_step / 1e6
+
+
 def get_workload(args, rank: int):
     import datagen
     w = datagen.WORKLOADS[args.workload]
@@ -220,11 +236,7 @@ def run_ours(args):
             dist.barrier()
 
     def max_over_ranks(v: float) -> float:
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_max_over_ranks(v, world, "cuda")
 
     import datagen
     import paper_1509_00186_b200 as dd          # raises if libdedisp.so is missing: no fallback
@@ -274,7 +286,7 @@ def run_ours(args):
         mark1 = sampler.mark()
     clocks = sampler.stop(mark0, max(mark1, mark0 + 1)) if sampler else None
     ms_step = ms_total / args.steps
-    value = world * samples / (ms_step * 1e-3) / 1e6
+    value = whole_job_value(samples, world, ms_step * 1e-3)
     checksum = float(d_out[:, :, : min(n_out, 1000)].double().mean().item())   # touches the result; sanity only
 
     # ---- end to end from pinned host memory (config 3: 1 s chunks, double buffered) -------------------------------
