@@ -28,6 +28,8 @@ static void free_plan(dedisp_plan_s* p)
     dedisp_stream_free(p);
     if (p->d_chirp) cudaFree(p->d_chirp);
     if (p->d_twiddle) cudaFree(p->d_twiddle);
+    if (p->d_chirp4) cudaFree(p->d_chirp4);
+    if (p->d_twiddle4) cudaFree(p->d_twiddle4);
     if (p->d_xt) cudaFree(p->d_xt);
     if (p->d_spec) cudaFree(p->d_spec);
     if (p->prof_ev) {
@@ -44,7 +46,8 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     if (!out_plan) return DEDISP_EINVAL;
     *out_plan = nullptr;
     if ((flags & ~DEDISP_TAPER_MASK) || (flags & DEDISP_TAPER_MASK) == 3u) return DEDISP_EINVAL;
-    if (n_fft <= 0 || (n_fft & (n_fft - 1)) || !dedisp_fused_supported(n_fft)) return DEDISP_EINVAL;
+    if (n_fft <= 0 || (n_fft & (n_fft - 1)) || !(dedisp_fused_supported(n_fft) || dedisp_pair_supported(n_fft)))
+        return DEDISP_EINVAL;
     // R9 gives D_tot % n_int == 0, so L % n_int == n_fft % n_int: only powers of two can divide a block evenly
     if (n_int <= 0 || (n_int & (n_int - 1))) return DEDISP_EINVAL;
     int head, tail, L;
@@ -88,16 +91,23 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
             return fail(e__ == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA);        \
         }                                                                                        \
     } while (0)
-    rc = dedisp_fused_init();
+    p->use_pair = dedisp_pair_supported(n_fft);
+    rc = p->use_pair ? dedisp_pair_init() : dedisp_fused_init();
     if (rc != DEDISP_OK) return fail(rc);
-    PLAN_TRY(cudaMalloc(&p->d_chirp, sizeof(float2) * (size_t)n_dm * n_chan * n_fft));
-    PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
-    if (n_dm > 1) PLAN_TRY(cudaMalloc(&p->d_spec, dedisp_fused_spec_bytes(n_fft)));
+    if (p->use_pair) {
+        PLAN_TRY(cudaMalloc(&p->d_chirp4, sizeof(float4) * (size_t)n_dm * n_chan * n_fft));
+        PLAN_TRY(cudaMalloc(&p->d_twiddle4, sizeof(float4) * (size_t)n_fft));
+    } else {
+        PLAN_TRY(cudaMalloc(&p->d_chirp, sizeof(float2) * (size_t)n_dm * n_chan * n_fft));
+        PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
+    }
+    if (n_dm > 1)
+        PLAN_TRY(cudaMalloc(&p->d_spec, p->use_pair ? dedisp_pair_spec_bytes(n_fft) : dedisp_fused_spec_bytes(n_fft)));
     PLAN_TRY(cudaMalloc(&d_dm, sizeof(double) * n_dm));
     PLAN_TRY(cudaMemcpy(d_dm, p->dm, sizeof(double) * n_dm, cudaMemcpyHostToDevice));
     rc = dedisp_launch_chirp_table(p, d_dm, 0);
     if (rc != DEDISP_OK) return fail(rc);
-    rc = dedisp_launch_twiddle_table(p->d_twiddle, n_fft, 0);
+    rc = dedisp_launch_twiddle_table(p, 0);
     if (rc != DEDISP_OK) return fail(rc);
     PLAN_TRY(cudaDeviceSynchronize());
     cudaFree(d_dm);
@@ -139,7 +149,8 @@ int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows,
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[1], st));
     if (after_corner_turn) DEDISP_CUDA_TRY(cudaEventRecord(after_corner_turn, st));
     if (nb > 0) {
-        rc = dedisp_launch_fused(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st);
+        rc = p->use_pair ? dedisp_launch_pair(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st)
+                         : dedisp_launch_fused(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st);
         if (rc != DEDISP_OK) return rc;
     }
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[2], st));
@@ -226,8 +237,15 @@ extern "C" int dedisp_destroy(dedisp_plan_t p)
 extern "C" int dedisp_debug_chirp(dedisp_plan_t p, int d, int chan, float* h_chirp)
 {
     if (!p || !h_chirp || d < 0 || d >= p->n_dm || chan < 0 || chan >= p->n_chan) return DEDISP_EINVAL;
-    DEDISP_CUDA_TRY(cudaMemcpy(h_chirp, p->d_chirp + ((size_t)d * p->n_chan + chan) * p->n_fft,
-                               sizeof(float2) * p->n_fft, cudaMemcpyDeviceToHost));
+    const size_t row = ((size_t)d * p->n_chan + chan) * p->n_fft;
+    if (p->use_pair) {  // (c, c, s, s) -> (c, s): columns 0 and 2 of the float4 row
+        DEDISP_CUDA_TRY(cudaMemcpy2D(h_chirp, sizeof(float2), p->d_chirp4 + row, sizeof(float4), sizeof(float),
+                                     p->n_fft, cudaMemcpyDeviceToHost));
+        DEDISP_CUDA_TRY(cudaMemcpy2D(h_chirp + 1, sizeof(float2), reinterpret_cast<const float*>(p->d_chirp4 + row) + 2,
+                                     sizeof(float4), sizeof(float), p->n_fft, cudaMemcpyDeviceToHost));
+        return DEDISP_OK;
+    }
+    DEDISP_CUDA_TRY(cudaMemcpy(h_chirp, p->d_chirp + row, sizeof(float2) * p->n_fft, cudaMemcpyDeviceToHost));
     return DEDISP_OK;
 }
 
@@ -260,5 +278,6 @@ extern "C" int dedisp_debug_voltage(dedisp_plan_t p, const int8_t* d_in, long lo
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = debug_prepare(p, d_in, n_samp, chan, block, st);
     if (rc != DEDISP_OK) return rc;
-    return dedisp_launch_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st);
+    return p->use_pair ? dedisp_launch_pair_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st)
+                       : dedisp_launch_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st);
 }

@@ -23,8 +23,13 @@ struct dedisp_plan_s {
     int nfft_rule;
     int device;
     // device tables owned by the plan
+    // n_fft <= 4096 runs the packed pair kernel (fused_pair.cu), which wants every table value in both f32x2 lanes:
+    // float4 (c, c, s, s); larger transforms run the scalar kernel (fused.cu) on float2 (c, s).  Only one set exists.
+    int use_pair;
     float2* d_chirp;    // [n_dm][n_chan][n_fft], taper * exp(+2 pi i psi) / n_fft
     float2* d_twiddle;  // [n_fft], exp(-2 pi i m / n_fft)
+    float4* d_chirp4;   // same values, pair layout
+    float4* d_twiddle4;
     // channel-major int8 scratch: [n_chan][xt_stride] (re,im) pairs, xt_stride samples per row
     float2* d_spec;     // [resident CTAs][units per CTA][n_fft] forward-spectrum stash shared by the trial DMs (n_dm > 1)
     int8_t* d_xt;
@@ -64,12 +69,20 @@ int dedisp_launch_debug_unpack(const dedisp_plan_s* p, const int8_t* d_xt, long 
                                long long block, float* d_block, cudaStream_t st);
 int dedisp_launch_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
                                 long long block, float* d_volt, cudaStream_t st);
+// fused_pair.cu: same contract as the three launchers above, for n_fft <= 4096
+int dedisp_launch_pair(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
+                       long long out_stride, long long out_col0, cudaStream_t st);
+int dedisp_launch_pair_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
+                                     long long block, float* d_volt, cudaStream_t st);
+int dedisp_pair_supported(int n_fft);
+size_t dedisp_pair_spec_bytes(int n_fft);
+int dedisp_pair_init(void);
 int dedisp_fused_supported(int n_fft);
 size_t dedisp_fused_spec_bytes(int n_fft);  // valid after dedisp_fused_init()
 int dedisp_fused_init(void);  // sets the dynamic shared memory attributes once per process
 // plan-time table generation on the device (fp64 phase)
 int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaStream_t st);
-int dedisp_launch_twiddle_table(float2* d_tw, int n_fft, cudaStream_t st);
+int dedisp_launch_twiddle_table(const dedisp_plan_s* p, cudaStream_t st);
 // framing (R9) with the largest in-band smear (samples) reported as well
 int dedisp_framing_impl(int n_chan, double bw, double F, const double* dm, int n_dm, int n_fft, int n_int, int* head,
                         int* tail, int* L, double* max_smear);

@@ -1,0 +1,198 @@
+// fft_pair.cuh -- register-resident Stockham FFT on PACKED pairs, for the sm_100 f32x2 instructions (FADD2/FMUL2/FFMA2).
+//
+// A thread holds 16 complex "slots"; each slot carries TWO independent complex numbers in the two lanes of a packed
+// float2: lane .x belongs to unit A, lane .y to unit B (two overlap-save blocks of the same channel).  Both units go
+// through identical butterflies with identical twiddles, so every FP32 instruction of the transform is a packed one:
+// half the issue slots of the scalar form for the same lane throughput (profiles/r1b_fp32_issue.md), and the index
+// arithmetic, twiddle loads and twiddle powers are shared by the two units.
+//
+// Indexing is the one of fft_regs.cuh: slot m of thread t is element i = t + m*TPU (TPU = N/16); a radix-R pass runs
+// S = 16/R butterflies per thread on slots q + r*S; after the last pass the spectrum is back in the same slot map.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace dedisp_pair {
+
+typedef float2 V;  // two fp32 lanes: (unit A, unit B)
+struct C2 { V re, im; };
+
+__device__ __forceinline__ V vdup(float a) { return make_float2(a, a); }
+__device__ __forceinline__ V vneg(V a) { return make_float2(-a.x, -a.y); }  // folds into operand modifiers
+__device__ __forceinline__ V vadd(V a, V b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ V vsub(V a, V b) { return __fadd2_rn(a, vneg(b)); }
+__device__ __forceinline__ V vmul(V a, V b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ V vfma(V a, V b, V c) { return __ffma2_rn(a, b, c); }
+
+__device__ __forceinline__ C2 cadd(C2 a, C2 b) { return C2{vadd(a.re, b.re), vadd(a.im, b.im)}; }
+__device__ __forceinline__ C2 csub(C2 a, C2 b) { return C2{vsub(a.re, b.re), vsub(a.im, b.im)}; }
+__device__ __forceinline__ C2 cmul(C2 a, C2 w)
+{
+    return C2{vfma(vneg(a.im), w.im, vmul(a.re, w.re)), vfma(a.im, w.re, vmul(a.re, w.im))};
+}
+__device__ __forceinline__ C2 csqr(C2 w)
+{
+    const V t = vmul(w.re, w.im);
+    return C2{vfma(vneg(w.im), w.im, vmul(w.re, w.re)), vadd(t, t)};
+}
+
+// d * exp(SIGN * 2*pi*i * j/16), j in [0, 8); j and SIGN are compile-time constants after unrolling.
+template <int SIGN>
+__device__ __forceinline__ C2 mul_w16(C2 d, int j)
+{
+    constexpr float s = (float)SIGN;
+    constexpr float C1 = 0.92387953251128674f;  // cos(pi/8)
+    constexpr float S1 = 0.38268343236508977f;  // sin(pi/8)
+    constexpr float H = 0.70710678118654752f;   // sqrt(1/2)
+    switch (j) {
+        case 0: return d;
+        case 1: return C2{vfma(d.im, vdup(-s * S1), vmul(d.re, vdup(C1))), vfma(d.re, vdup(s * S1), vmul(d.im, vdup(C1)))};
+        case 2: return SIGN > 0 ? C2{vmul(vsub(d.re, d.im), vdup(H)), vmul(vadd(d.re, d.im), vdup(H))}
+                                : C2{vmul(vadd(d.re, d.im), vdup(H)), vmul(vsub(d.im, d.re), vdup(H))};
+        case 3: return C2{vfma(d.im, vdup(-s * C1), vmul(d.re, vdup(S1))), vfma(d.re, vdup(s * C1), vmul(d.im, vdup(S1)))};
+        case 4: return SIGN > 0 ? C2{vneg(d.im), d.re} : C2{d.im, vneg(d.re)};
+        case 5: return C2{vfma(d.im, vdup(-s * C1), vmul(d.re, vdup(-S1))), vfma(d.re, vdup(s * C1), vmul(d.im, vdup(-S1)))};
+        case 6: return SIGN > 0 ? C2{vmul(vadd(d.re, d.im), vdup(-H)), vmul(vsub(d.re, d.im), vdup(H))}
+                                : C2{vmul(vsub(d.im, d.re), vdup(H)), vmul(vadd(d.re, d.im), vdup(-H))};
+        default: return C2{vfma(d.im, vdup(-s * S1), vmul(d.re, vdup(-C1))), vfma(d.re, vdup(s * S1), vmul(d.im, vdup(-C1)))};
+    }
+}
+
+__host__ __device__ constexpr int bitrev(int r, int R)
+{
+    int o = 0;
+    for (int b = 1; b < R; b <<= 1) { o = (o << 1) | (r & 1); r >>= 1; }
+    return o;
+}
+
+// In-register radix-R DFT (decimation in frequency) on slots q + r*S; X[r] ends up in slot q + bitrev(r)*S.
+template <int R, int SIGN>
+__device__ __forceinline__ void butterfly(C2 (&x)[16], int q)
+{
+    constexpr int S = 16 / R;
+#pragma unroll
+    for (int half = R / 2; half >= 1; half >>= 1) {
+#pragma unroll
+        for (int g = 0; g < R; g += 2 * half) {
+#pragma unroll
+            for (int k = 0; k < half; ++k) {
+                const C2 u = x[q + (g + k) * S], w = x[q + (g + k + half) * S];
+                x[q + (g + k) * S] = cadd(u, w);
+                x[q + (g + k + half) * S] = mul_w16<SIGN>(csub(u, w), k * (8 / half));
+            }
+        }
+    }
+}
+
+// x[q + r*S] *= w1^r, r = 1..R-1.  Powers by products of depth <= log2 R; ordered so that at most w1,w2,w3,w4,w8 and
+// one temporary are alive at a time.
+template <int R>
+__device__ __forceinline__ void twiddle(C2 (&x)[16], int q, C2 w1)
+{
+    constexpr int S = 16 / R;
+#define XR(r) x[q + (r) * S]
+    XR(1) = cmul(XR(1), w1);
+    if constexpr (R >= 4) {
+        const C2 w2 = csqr(w1);
+        const C2 w3 = cmul(w2, w1);
+        XR(2) = cmul(XR(2), w2);
+        XR(3) = cmul(XR(3), w3);
+        if constexpr (R >= 8) {
+            const C2 w4 = csqr(w2);
+            XR(4) = cmul(XR(4), w4);
+            XR(5) = cmul(XR(5), cmul(w4, w1));
+            XR(6) = cmul(XR(6), cmul(w4, w2));
+            XR(7) = cmul(XR(7), cmul(w4, w3));
+            if constexpr (R >= 16) {
+                const C2 w8 = csqr(w4);
+                XR(8) = cmul(XR(8), w8);
+                XR(9) = cmul(XR(9), cmul(w8, w1));
+                XR(10) = cmul(XR(10), cmul(w8, w2));
+                XR(11) = cmul(XR(11), cmul(w8, w3));
+                XR(12) = cmul(XR(12), cmul(w8, w4));
+                const C2 w12 = cmul(w8, w4);
+                XR(13) = cmul(XR(13), cmul(w12, w1));
+                XR(14) = cmul(XR(14), cmul(w12, w2));
+                XR(15) = cmul(XR(15), cmul(w12, w3));
+            }
+        }
+    }
+#undef XR
+}
+
+// One 16-byte cell of padding per 16 keeps the strided STS.128 of an exchange (stride R*NS cells) and its contiguous
+// LDS.128 free of bank conflicts (a 128-bit access is served 8 lanes at a time).
+__device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
+__host__ __device__ constexpr int padded_len(int n) { return n + (n >> 4); }
+
+// One pass: twiddle (skipped when NS == 1) + butterflies.  tw4[m] = (c, c, s, s), c + i s = exp(-2*pi*i*m/N).
+template <int N, int R, int NS, int SIGN>
+__device__ __forceinline__ void pass_compute(C2 (&x)[16], int t, const float4* __restrict__ tw4)
+{
+    constexpr int S = 16 / R;
+    constexpr int TPU = N / 16;
+#pragma unroll
+    for (int q = 0; q < S; ++q) {
+        if (NS > 1) {
+            const int k = (t + q * TPU) & (NS - 1);
+            const float4 w = __ldg(&tw4[k * (N / (NS * R))]);
+            C2 w1{make_float2(w.x, w.y), make_float2(w.z, w.w)};
+            if (SIGN > 0) w1.im = vneg(w1.im);
+            twiddle<R>(x, q, w1);
+        }
+        butterfly<R, SIGN>(x, q);
+    }
+}
+
+// Exchange through shared memory in (reA, reB, imA, imB) cells: scatter to the Stockham positions, gather the next map.
+template <int N, int R, int NS>
+__device__ __forceinline__ void exchange(C2 (&x)[16], int t, float4* __restrict__ sm)
+{
+    constexpr int S = 16 / R;
+    constexpr int TPU = N / 16;
+#pragma unroll
+    for (int q = 0; q < S; ++q) {
+        const int jv = t + q * TPU;
+        const int k = jv & (NS - 1);
+        const int j0 = (jv - k) * R + k;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const C2 v = x[q + bitrev(r, R) * S];
+            sm[pad16(j0 + r * NS)] = make_float4(v.re.x, v.re.y, v.im.x, v.im.y);
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int m = 0; m < 16; ++m) {
+        const float4 v = sm[pad16(t + m * TPU)];
+        x[m] = C2{make_float2(v.x, v.y), make_float2(v.z, v.w)};
+    }
+    __syncthreads();
+}
+
+// Puts the outputs of a final radix-R pass (left bit-reversed by butterfly()) back into the canonical slot map.
+template <int R>
+__device__ __forceinline__ void natural_order(C2 (&x)[16])
+{
+    constexpr int S = 16 / R;
+    C2 y[16];
+#pragma unroll
+    for (int q = 0; q < S; ++q)
+#pragma unroll
+        for (int r = 0; r < R; ++r) y[q + r * S] = x[q + bitrev(r, R) * S];
+#pragma unroll
+    for (int m = 0; m < 16; ++m) x[m] = y[m];
+}
+
+// Full N-point transform (N = R0*R1*R2) of both lanes; unnormalised; kernel exp(SIGN*2*pi*i*k*n/N).
+template <int N, int R0, int R1, int R2, int SIGN>
+__device__ __forceinline__ void fft_pair(C2 (&x)[16], int t, float4* __restrict__ sm, const float4* __restrict__ tw4)
+{
+    pass_compute<N, R0, 1, SIGN>(x, t, tw4);
+    exchange<N, R0, 1>(x, t, sm);
+    pass_compute<N, R1, R0, SIGN>(x, t, tw4);
+    exchange<N, R1, R0>(x, t, sm);
+    pass_compute<N, R2, R0 * R1, SIGN>(x, t, tw4);
+    natural_order<R2>(x);
+}
+
+}  // namespace dedisp_pair
