@@ -28,7 +28,6 @@ static void free_plan(dedisp_plan_s* p)
     dedisp_stream_free(p);
     if (p->d_chirp) cudaFree(p->d_chirp);
     if (p->d_twiddle) cudaFree(p->d_twiddle);
-    if (p->d_chirp4) cudaFree(p->d_chirp4);
     if (p->d_twiddle4) cudaFree(p->d_twiddle4);
     if (p->d_xt) cudaFree(p->d_xt);
     if (p->d_spec) cudaFree(p->d_spec);
@@ -94,13 +93,9 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     p->use_pair = dedisp_pair_supported(n_fft);
     rc = p->use_pair ? dedisp_pair_init() : dedisp_fused_init();
     if (rc != DEDISP_OK) return fail(rc);
-    if (p->use_pair) {
-        PLAN_TRY(cudaMalloc(&p->d_chirp4, sizeof(float4) * (size_t)n_dm * n_chan * n_fft));
-        PLAN_TRY(cudaMalloc(&p->d_twiddle4, sizeof(float4) * (size_t)n_fft));
-    } else {
-        PLAN_TRY(cudaMalloc(&p->d_chirp, sizeof(float2) * (size_t)n_dm * n_chan * n_fft));
-        PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
-    }
+    PLAN_TRY(cudaMalloc(&p->d_chirp, sizeof(float2) * (size_t)n_dm * n_chan * n_fft));
+    if (p->use_pair) PLAN_TRY(cudaMalloc(&p->d_twiddle4, sizeof(float4) * (size_t)n_fft));
+    else PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
     if (n_dm > 1)
         PLAN_TRY(cudaMalloc(&p->d_spec, p->use_pair ? dedisp_pair_spec_bytes(n_fft) : dedisp_fused_spec_bytes(n_fft)));
     PLAN_TRY(cudaMalloc(&d_dm, sizeof(double) * n_dm));
@@ -238,13 +233,6 @@ extern "C" int dedisp_debug_chirp(dedisp_plan_t p, int d, int chan, float* h_chi
 {
     if (!p || !h_chirp || d < 0 || d >= p->n_dm || chan < 0 || chan >= p->n_chan) return DEDISP_EINVAL;
     const size_t row = ((size_t)d * p->n_chan + chan) * p->n_fft;
-    if (p->use_pair) {  // (c, c, s, s) -> (c, s): columns 0 and 2 of the float4 row
-        DEDISP_CUDA_TRY(cudaMemcpy2D(h_chirp, sizeof(float2), p->d_chirp4 + row, sizeof(float4), sizeof(float),
-                                     p->n_fft, cudaMemcpyDeviceToHost));
-        DEDISP_CUDA_TRY(cudaMemcpy2D(h_chirp + 1, sizeof(float2), reinterpret_cast<const float*>(p->d_chirp4 + row) + 2,
-                                     sizeof(float4), sizeof(float), p->n_fft, cudaMemcpyDeviceToHost));
-        return DEDISP_OK;
-    }
     DEDISP_CUDA_TRY(cudaMemcpy(h_chirp, p->d_chirp + row, sizeof(float2) * p->n_fft, cudaMemcpyDeviceToHost));
     return DEDISP_OK;
 }

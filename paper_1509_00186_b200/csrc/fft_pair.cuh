@@ -143,9 +143,11 @@ __device__ __forceinline__ void pass_compute(C2 (&x)[16], int t, const float4* _
     }
 }
 
-// Exchange through shared memory in (reA, reB, imA, imB) cells: scatter to the Stockham positions, gather the next map.
+// Exchange through shared memory in (reA, reB, imA, imB) cells, in two halves so that the caller can place its barrier
+// (and work that only needs the barrier, like a prefetch) between them: scatter the pass outputs to their Stockham
+// positions; [barrier]; gather the next slot map; [barrier before the buffer is written again].
 template <int N, int R, int NS>
-__device__ __forceinline__ void exchange(C2 (&x)[16], int t, float4* __restrict__ sm)
+__device__ __forceinline__ void exchange_scatter(const C2 (&x)[16], int t, float4* __restrict__ sm)
 {
     constexpr int S = 16 / R;
     constexpr int TPU = N / 16;
@@ -160,13 +162,23 @@ __device__ __forceinline__ void exchange(C2 (&x)[16], int t, float4* __restrict_
             sm[pad16(j0 + r * NS)] = make_float4(v.re.x, v.re.y, v.im.x, v.im.y);
         }
     }
-    __syncthreads();
+}
+
+template <int N>
+__device__ __forceinline__ void exchange_gather(C2 (&x)[16], int t, const float4* __restrict__ sm)
+{
+    constexpr int TPU = N / 16;
 #pragma unroll
     for (int m = 0; m < 16; ++m) {
         const float4 v = sm[pad16(t + m * TPU)];
         x[m] = C2{make_float2(v.x, v.y), make_float2(v.z, v.w)};
     }
-    __syncthreads();
+}
+
+// Named barrier over the `count` threads that share one exchange buffer (ids 1..15; 0 is __syncthreads).
+__device__ __forceinline__ void group_bar(int id, int count)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
 }
 
 // Puts the outputs of a final radix-R pass (left bit-reversed by butterfly()) back into the canonical slot map.
@@ -183,14 +195,23 @@ __device__ __forceinline__ void natural_order(C2 (&x)[16])
     for (int m = 0; m < 16; ++m) x[m] = y[m];
 }
 
-// Full N-point transform (N = R0*R1*R2) of both lanes; unnormalised; kernel exp(SIGN*2*pi*i*k*n/N).
-template <int N, int R0, int R1, int R2, int SIGN>
-__device__ __forceinline__ void fft_pair(C2 (&x)[16], int t, float4* __restrict__ sm, const float4* __restrict__ tw4)
+// Full N-point transform (N = R0*R1*R2) of both lanes; unnormalised; kernel exp(SIGN*2*pi*i*k*n/N).  `after_first`
+// runs once between the first barrier and the first gather (the fused kernel issues its input prefetch there).
+template <int N, int R0, int R1, int R2, int SIGN, class F>
+__device__ __forceinline__ void fft_pair(C2 (&x)[16], int t, float4* __restrict__ sm, const float4* __restrict__ tw4,
+                                         int bar_id, int bar_count, F after_first)
 {
     pass_compute<N, R0, 1, SIGN>(x, t, tw4);
-    exchange<N, R0, 1>(x, t, sm);
+    exchange_scatter<N, R0, 1>(x, t, sm);
+    group_bar(bar_id, bar_count);
+    after_first();
+    exchange_gather<N>(x, t, sm);
+    group_bar(bar_id, bar_count);
     pass_compute<N, R1, R0, SIGN>(x, t, tw4);
-    exchange<N, R1, R0>(x, t, sm);
+    exchange_scatter<N, R1, R0>(x, t, sm);
+    group_bar(bar_id, bar_count);
+    exchange_gather<N>(x, t, sm);
+    group_bar(bar_id, bar_count);
     pass_compute<N, R2, R0 * R1, SIGN>(x, t, tw4);
     natural_order<R2>(x);
 }

@@ -72,9 +72,8 @@ extern "C" int dedisp_framing(int n_chan, double bw_hz, double f_center_hz, cons
 // Plan-time tables, generated on the device with the phase in fp64
 // ---------------------------------------------------------------------------------------------------------------
 // chirp[d][c][k] = w(f_k) * exp(+2 pi i psi) / N,  psi = D DM f^2 / ((f + f_c) f_c^2) cycles (Eq. 3; R1, R2)
-__global__ void chirp_table_kernel(float2* __restrict__ chirp, float4* __restrict__ chirp4,
-                                   const double* __restrict__ dm, int n_chan, int n_fft, double bw, double F,
-                                   unsigned taper)
+__global__ void chirp_table_kernel(float2* __restrict__ chirp, const double* __restrict__ dm, int n_chan, int n_fft,
+                                   double bw, double F, unsigned taper)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int c = blockIdx.y, d = blockIdx.z;
@@ -95,10 +94,7 @@ __global__ void chirp_table_kernel(float2* __restrict__ chirp, float4* __restric
         const double r = 2.0 * f / dv;
         w *= 1.0 - r * r;
     }
-    const size_t at = ((size_t)d * n_chan + c) * n_fft + k;
-    const float re = (float)(w * co), im = (float)(w * s);
-    if (chirp4) chirp4[at] = make_float4(re, re, im, im);
-    else chirp[at] = make_float2(re, im);
+    chirp[((size_t)d * n_chan + c) * n_fft + k] = make_float2((float)(w * co), (float)(w * s));
 }
 
 __global__ void twiddle_table_kernel(float2* __restrict__ tw, float4* __restrict__ tw4, int n_fft)
@@ -114,7 +110,7 @@ __global__ void twiddle_table_kernel(float2* __restrict__ tw, float4* __restrict
 int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaStream_t st)
 {
     dim3 grid((p->n_fft + 255) / 256, p->n_chan, p->n_dm);
-    chirp_table_kernel<<<grid, 256, 0, st>>>(p->d_chirp, p->d_chirp4, d_dm, p->n_chan, p->n_fft, p->bw_hz, p->f_center_hz,
+    chirp_table_kernel<<<grid, 256, 0, st>>>(p->d_chirp, d_dm, p->n_chan, p->n_fft, p->bw_hz, p->f_center_hz,
                                              p->flags & DEDISP_TAPER_MASK);
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;
