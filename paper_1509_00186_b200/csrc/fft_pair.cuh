@@ -83,40 +83,81 @@ __device__ __forceinline__ void butterfly(C2 (&x)[16], int q)
     }
 }
 
-// x[q + r*S] *= w1^r, r = 1..R-1.  Powers by products of depth <= log2 R; ordered so that at most w1,w2,w3,w4,w8 and
-// one temporary are alive at a time.
-template <int R>
-__device__ __forceinline__ void twiddle(C2 (&x)[16], int q, C2 w1)
+// Twiddles of one pass, in two steps so that the serial part (table load, squarings) runs in the window between the
+// scatter and the gather of the preceding exchange, where the 64 data registers are dead and the thread would
+// otherwise wait at the barrier:  prepare = w1 (and for radix 16 the powers 2, 3, 4, 8, 12);  apply = the remaining
+// products and x[q + r*S] *= w1^r, r = 1..R-1.  Every power is a product of depth <= log2 R.
+template <int R> struct TwSet { C2 w1[16 / R]; };
+template <> struct TwSet<16> { C2 w1, w2, w3, w4, w8, w12; };
+
+template <int N, int R, int NS, int SIGN>
+__device__ __forceinline__ TwSet<R> twiddle_prepare(int t, const float4* __restrict__ tw4)
 {
     constexpr int S = 16 / R;
-#define XR(r) x[q + (r) * S]
-    XR(1) = cmul(XR(1), w1);
-    if constexpr (R >= 4) {
-        const C2 w2 = csqr(w1);
-        const C2 w3 = cmul(w2, w1);
-        XR(2) = cmul(XR(2), w2);
-        XR(3) = cmul(XR(3), w3);
-        if constexpr (R >= 8) {
-            const C2 w4 = csqr(w2);
-            XR(4) = cmul(XR(4), w4);
-            XR(5) = cmul(XR(5), cmul(w4, w1));
-            XR(6) = cmul(XR(6), cmul(w4, w2));
-            XR(7) = cmul(XR(7), cmul(w4, w3));
-            if constexpr (R >= 16) {
-                const C2 w8 = csqr(w4);
-                XR(8) = cmul(XR(8), w8);
-                XR(9) = cmul(XR(9), cmul(w8, w1));
-                XR(10) = cmul(XR(10), cmul(w8, w2));
-                XR(11) = cmul(XR(11), cmul(w8, w3));
-                XR(12) = cmul(XR(12), cmul(w8, w4));
-                const C2 w12 = cmul(w8, w4);
-                XR(13) = cmul(XR(13), cmul(w12, w1));
-                XR(14) = cmul(XR(14), cmul(w12, w2));
-                XR(15) = cmul(XR(15), cmul(w12, w3));
-            }
+    constexpr int TPU = N / 16;
+    TwSet<R> tw;
+    if constexpr (R == 16) {
+        const float4 w = __ldg(&tw4[(t & (NS - 1)) * (N / (NS * R))]);
+        tw.w1 = C2{make_float2(w.x, w.y), make_float2(w.z, w.w)};
+        if (SIGN > 0) tw.w1.im = vneg(tw.w1.im);
+        tw.w2 = csqr(tw.w1);
+        tw.w3 = cmul(tw.w2, tw.w1);
+        tw.w4 = csqr(tw.w2);
+        tw.w8 = csqr(tw.w4);
+        tw.w12 = cmul(tw.w8, tw.w4);
+    } else {
+#pragma unroll
+        for (int q = 0; q < S; ++q) {
+            const float4 w = __ldg(&tw4[((t + q * TPU) & (NS - 1)) * (N / (NS * R))]);
+            tw.w1[q] = C2{make_float2(w.x, w.y), make_float2(w.z, w.w)};
+            if (SIGN > 0) tw.w1[q].im = vneg(tw.w1[q].im);
         }
     }
+    return tw;
+}
+
+template <int R>
+__device__ __forceinline__ void twiddle_apply(C2 (&x)[16], const TwSet<R>& tw)
+{
+    constexpr int S = 16 / R;
+    if constexpr (R == 16) {
+        x[1] = cmul(x[1], tw.w1);
+        x[2] = cmul(x[2], tw.w2);
+        x[3] = cmul(x[3], tw.w3);
+        x[4] = cmul(x[4], tw.w4);
+        x[5] = cmul(x[5], cmul(tw.w4, tw.w1));
+        x[6] = cmul(x[6], cmul(tw.w4, tw.w2));
+        x[7] = cmul(x[7], cmul(tw.w4, tw.w3));
+        x[8] = cmul(x[8], tw.w8);
+        x[9] = cmul(x[9], cmul(tw.w8, tw.w1));
+        x[10] = cmul(x[10], cmul(tw.w8, tw.w2));
+        x[11] = cmul(x[11], cmul(tw.w8, tw.w3));
+        x[12] = cmul(x[12], tw.w12);
+        x[13] = cmul(x[13], cmul(tw.w12, tw.w1));
+        x[14] = cmul(x[14], cmul(tw.w12, tw.w2));
+        x[15] = cmul(x[15], cmul(tw.w12, tw.w3));
+    } else {
+#pragma unroll
+        for (int q = 0; q < S; ++q) {
+#define XR(r) x[q + (r) * S]
+            const C2 w1 = tw.w1[q];
+            XR(1) = cmul(XR(1), w1);
+            if constexpr (R >= 4) {
+                const C2 w2 = csqr(w1);
+                const C2 w3 = cmul(w2, w1);
+                XR(2) = cmul(XR(2), w2);
+                XR(3) = cmul(XR(3), w3);
+                if constexpr (R >= 8) {
+                    const C2 w4 = csqr(w2);
+                    XR(4) = cmul(XR(4), w4);
+                    XR(5) = cmul(XR(5), cmul(w4, w1));
+                    XR(6) = cmul(XR(6), cmul(w4, w2));
+                    XR(7) = cmul(XR(7), cmul(w4, w3));
+                }
+            }
 #undef XR
+        }
+    }
 }
 
 // One 16-byte cell of padding per 16 keeps the strided STS.128 of an exchange (stride R*NS cells) and its contiguous
@@ -124,23 +165,12 @@ __device__ __forceinline__ void twiddle(C2 (&x)[16], int q, C2 w1)
 __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
 __host__ __device__ constexpr int padded_len(int n) { return n + (n >> 4); }
 
-// One pass: twiddle (skipped when NS == 1) + butterflies.  tw4[m] = (c, c, s, s), c + i s = exp(-2*pi*i*m/N).
-template <int N, int R, int NS, int SIGN>
-__device__ __forceinline__ void pass_compute(C2 (&x)[16], int t, const float4* __restrict__ tw4)
+// The butterflies of one pass (after twiddle_apply when NS > 1).
+template <int R, int SIGN>
+__device__ __forceinline__ void pass_butterflies(C2 (&x)[16])
 {
-    constexpr int S = 16 / R;
-    constexpr int TPU = N / 16;
 #pragma unroll
-    for (int q = 0; q < S; ++q) {
-        if (NS > 1) {
-            const int k = (t + q * TPU) & (NS - 1);
-            const float4 w = __ldg(&tw4[k * (N / (NS * R))]);
-            C2 w1{make_float2(w.x, w.y), make_float2(w.z, w.w)};
-            if (SIGN > 0) w1.im = vneg(w1.im);
-            twiddle<R>(x, q, w1);
-        }
-        butterfly<R, SIGN>(x, q);
-    }
+    for (int q = 0; q < 16 / R; ++q) butterfly<R, SIGN>(x, q);
 }
 
 // Exchange through shared memory in (reA, reB, imA, imB) cells, in two halves so that the caller can place its barrier
@@ -151,15 +181,25 @@ __device__ __forceinline__ void exchange_scatter(const C2 (&x)[16], int t, float
 {
     constexpr int S = 16 / R;
     constexpr int TPU = N / 16;
+    static_assert(NS == 1 ? R == 16 : NS % 16 == 0, "pad16(j0 + r*NS) must split into pad16(j0) + constant");
+    // j0 is a multiple of 16 when NS == 1 (and r < 16); r*NS is a multiple of 16 otherwise: either way the padded
+    // position of output r is pad16(j0) plus a compile-time constant, so every store is base + immediate.
+    constexpr int STEP = NS == 1 ? 1 : NS + NS / 16;
 #pragma unroll
     for (int q = 0; q < S; ++q) {
         const int jv = t + q * TPU;
         const int k = jv & (NS - 1);
-        const int j0 = (jv - k) * R + k;
+        const unsigned base = (unsigned)__cvta_generic_to_shared(sm + pad16((jv - k) * R + k));
 #pragma unroll
         for (int r = 0; r < R; ++r) {
+            // two 8-byte stores written in asm: the (re, im) register pairs of a slot are rarely adjacent, and nvcc
+            // would pay four register moves to build a 16-byte store (ptxas still pairs them when they are adjacent,
+            // and folds the constant address increments into the immediate offset)
             const C2 v = x[q + bitrev(r, R) * S];
-            sm[pad16(j0 + r * NS)] = make_float4(v.re.x, v.re.y, v.im.x, v.im.y);
+            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(base + 16 * r * STEP), "f"(v.re.x), "f"(v.re.y)
+                         : "memory");
+            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(base + 16 * r * STEP + 8), "f"(v.im.x), "f"(v.im.y)
+                         : "memory");
         }
     }
 }
@@ -167,10 +207,11 @@ __device__ __forceinline__ void exchange_scatter(const C2 (&x)[16], int t, float
 template <int N>
 __device__ __forceinline__ void exchange_gather(C2 (&x)[16], int t, const float4* __restrict__ sm)
 {
-    constexpr int TPU = N / 16;
+    constexpr int TPU = N / 16;  // a multiple of 16: pad16(t + m*TPU) = pad16(t) + m*(TPU + TPU/16)
+    const float4* base = sm + pad16(t);
 #pragma unroll
     for (int m = 0; m < 16; ++m) {
-        const float4 v = sm[pad16(t + m * TPU)];
+        const float4 v = base[m * (TPU + TPU / 16)];
         x[m] = C2{make_float2(v.x, v.y), make_float2(v.z, v.w)};
     }
 }
@@ -201,18 +242,22 @@ template <int N, int R0, int R1, int R2, int SIGN, class F>
 __device__ __forceinline__ void fft_pair(C2 (&x)[16], int t, float4* __restrict__ sm, const float4* __restrict__ tw4,
                                          int bar_id, int bar_count, F after_first)
 {
-    pass_compute<N, R0, 1, SIGN>(x, t, tw4);
+    pass_butterflies<R0, SIGN>(x);
     exchange_scatter<N, R0, 1>(x, t, sm);
+    const TwSet<R1> tw1 = twiddle_prepare<N, R1, R0, SIGN>(t, tw4);  // tw4[m] = (c, c, s, s) of exp(-2*pi*i*m/N)
     group_bar(bar_id, bar_count);
     after_first();
     exchange_gather<N>(x, t, sm);
     group_bar(bar_id, bar_count);
-    pass_compute<N, R1, R0, SIGN>(x, t, tw4);
+    twiddle_apply<R1>(x, tw1);
+    pass_butterflies<R1, SIGN>(x);
     exchange_scatter<N, R1, R0>(x, t, sm);
+    const TwSet<R2> tw2 = twiddle_prepare<N, R2, R0 * R1, SIGN>(t, tw4);
     group_bar(bar_id, bar_count);
     exchange_gather<N>(x, t, sm);
     group_bar(bar_id, bar_count);
-    pass_compute<N, R2, R0 * R1, SIGN>(x, t, tw4);
+    twiddle_apply<R2>(x, tw2);
+    pass_butterflies<R2, SIGN>(x);
     natural_order<R2>(x);
 }
 

@@ -50,6 +50,19 @@ __device__ __forceinline__ int pw_cell(int cell)
     return ((u ^ ((u >> 3) & 1)) << 1) | (cell & 1);
 }
 
+// byte `sel & 3` of w under the exponent byte of k = 0x4B000000: the fp32 number 2^23 + byte
+__device__ __forceinline__ float byte_to_f32_biased(uint32_t w, uint32_t k, int sel)
+{
+    uint32_t r;
+    switch (sel) {
+        case 0: asm("prmt.b32 %0, %1, %2, 0x7440;" : "=r"(r) : "r"(w), "r"(k)); break;
+        case 1: asm("prmt.b32 %0, %1, %2, 0x7441;" : "=r"(r) : "r"(w), "r"(k)); break;
+        case 2: asm("prmt.b32 %0, %1, %2, 0x7442;" : "=r"(r) : "r"(w), "r"(k)); break;
+        default: asm("prmt.b32 %0, %1, %2, 0x7443;" : "=r"(r) : "r"(w), "r"(k)); break;
+    }
+    return __uint_as_float(r);
+}
+
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -63,7 +76,8 @@ template <int N> constexpr size_t smem_bytes()
     return (size_t)GROUPS * PShape<N>::P * (sizeof(float4) * padded_len(N) + 2 * N * sizeof(uint16_t)) + sizeof(float2) * N;
 }
 
-template <int N>
+// LGN = log2(n_int) when it is one of the specialised values (the epilogue then has no run-time geometry), else -1.
+template <int N, int LGN>
 __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const PairArgs a)
 {
     using Sh = PShape<N>;
@@ -79,12 +93,12 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
     uint16_t* stage = reinterpret_cast<uint16_t*>(chirp_s + N) + (size_t)ps * 2 * N;   // [2][N] int8 pairs: A, B
     const uint16_t* xt16 = reinterpret_cast<const uint16_t*>(a.xt);
 
-    const int n_int = 1 << a.log2_nint;
-    const int n_out = a.L >> a.log2_nint;
-    // epilogue geometry: each lane sums `chunk` consecutive samples, `lpo` lanes make one output
-    const int chunk = n_int < 4 ? n_int : (n_int > 128 ? n_int / 32 : 4);
-    const int lpo = n_int / chunk;
-    const int n_work = a.L / chunk;
+    const int lgn = LGN >= 0 ? LGN : a.log2_nint;
+    const int n_out = a.L >> lgn;
+    // epilogue geometry: each lane sums 2^lg_chunk consecutive samples, 2^lg_lpo lanes make one output
+    const int lg_chunk = lgn < 2 ? lgn : (lgn > 7 ? lgn - 5 : 2);
+    const int lg_lpo = lgn - lg_chunk;
+    const int n_work = a.L >> lg_chunk;
 
     const int s_begin = a.first_super + (int)((long long)blockIdx.x * a.n_super / gridDim.x);
     const int s_end = a.first_super + (int)((long long)(blockIdx.x + 1) * a.n_super / gridDim.x);
@@ -135,10 +149,8 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
             const uint32_t vA = live ? (uint32_t)stage[t + m * TPU] : 0u;
             const uint32_t vB = liveB ? (uint32_t)stage[N + t + m * TPU] : 0u;
             const uint32_t w = __byte_perm(vA, vB, 0x5410) ^ 0x80808080u;  // (A.re, A.im, B.re, B.im) + 128
-            const V re = make_float2(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7440)),
-                                     __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7442)));
-            const V im = make_float2(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7441)),
-                                     __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7443)));
+            const V re = make_float2(byte_to_f32_biased(w, 0x4B000000u, 0), byte_to_f32_biased(w, 0x4B000000u, 2));
+            const V im = make_float2(byte_to_f32_biased(w, 0x4B000000u, 1), byte_to_f32_biased(w, 0x4B000000u, 3));
             x[m].re = vadd(re, vdup(-8388736.0f));
             x[m].im = vadd(im, vdup(-8388736.0f));
         }
@@ -195,38 +207,39 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
                 continue;
             }
             // 5 + 6. discard the overlap, detect, integrate n_int samples (R9, R11)
+            {
+                float2* cell = smp + pw_cell(t);  // TPU/2 is a multiple of 16 units: pw_cell(t + m*TPU) = pw_cell(t) + m*TPU
 #pragma unroll
-            for (int m = 0; m < 16; ++m)
-                smp[pw_cell(t + m * TPU)] = vfma(x[m].re, x[m].re, vmul(x[m].im, x[m].im));
+                for (int m = 0; m < 16; ++m) cell[m * TPU] = vfma(x[m].re, x[m].re, vmul(x[m].im, x[m].im));
+            }
             group_bar(bar_id, GROUP);
             float* dstA = a.out + ((size_t)d * a.n_chan + c) * a.out_stride + a.out_col0 + (long long)bA * n_out;
             float* dstB = dstA + n_out;
-            for (int base = 0; base < n_work; base += TPU) {  // uniform trip count: the shuffles need whole warps
-                const int id = base + t;
+            for (int id = t; id - t < n_work; id += TPU) {  // uniform trip count: the shuffles need whole warps
                 V acc = make_float2(0.f, 0.f);
                 if (id < n_work) {
-                    const int cell0 = a.head + id * chunk;
-                    if (chunk >= 4) {
-                        for (int j = 0; j < chunk; j += 4) {
+                    const int cell0 = a.head + (id << lg_chunk);
+                    if (lg_chunk >= 2) {
+                        for (int j = 0; j < (1 << lg_chunk); j += 4) {
                             const float4 u0 = *reinterpret_cast<const float4*>(&smp[pw_cell(cell0 + j)]);
                             const float4 u1 = *reinterpret_cast<const float4*>(&smp[pw_cell(cell0 + j + 2)]);
                             const V s0 = vadd(make_float2(u0.x, u0.y), make_float2(u0.z, u0.w));
                             const V s1 = vadd(make_float2(u1.x, u1.y), make_float2(u1.z, u1.w));
                             acc = vadd(acc, vadd(s0, s1));
                         }
-                    } else if (chunk == 2) {
+                    } else if (lg_chunk == 1) {
                         const float4 u0 = *reinterpret_cast<const float4*>(&smp[pw_cell(cell0)]);
                         acc = vadd(make_float2(u0.x, u0.y), make_float2(u0.z, u0.w));
                     } else {
                         acc = smp[pw_cell(cell0)];
                     }
                 }
-                for (int off = 1; off < lpo; off <<= 1) {
+                for (int off = 1; off < (1 << lg_lpo); off <<= 1) {
                     acc.x += __shfl_xor_sync(0xffffffffu, acc.x, off);
                     acc.y += __shfl_xor_sync(0xffffffffu, acc.y, off);
                 }
-                if (id < n_work && (id & (lpo - 1)) == 0) {
-                    const int o = id / lpo;
+                if (id < n_work && (id & ((1 << lg_lpo) - 1)) == 0) {
+                    const int o = id >> lg_lpo;
                     if (live) dstA[o] = acc.x;
                     if (liveB) dstB[o] = acc.y;
                 }
@@ -244,10 +257,16 @@ int slot_of(int n_fft) { return n_fft == 1024 ? 0 : n_fft == 2048 ? 1 : n_fft ==
 
 template <int N> int init_one(int slot)
 {
-    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_pair_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_pair_kernel<N, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem_bytes<N>()));
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_pair_kernel<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem_bytes<N>()));
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_pair_kernel<N, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem_bytes<N>()));
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_pair_kernel<N, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem_bytes<N>()));
     int occ = 0;
-    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_pair_kernel<N>, GROUP * GROUPS,
+    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_pair_kernel<N, -1>, GROUP * GROUPS,
                                                                   smem_bytes<N>()));
     int dev = 0, n_sm = 0;
     DEDISP_CUDA_TRY(cudaGetDevice(&dev));
@@ -265,7 +284,13 @@ int launch_one(const dedisp_plan_s* p, PairArgs& a, cudaStream_t st)
     long long grid = (long long)g_info[slot].ctas_per_sm * g_info[slot].n_sm;
     if (grid > a.n_super) grid = a.n_super;
     a.spec = reinterpret_cast<float4*>(p->d_spec);
-    fused_pair_kernel<N><<<(unsigned)grid, GROUP * GROUPS, smem_bytes<N>(), st>>>(a);
+    const dim3 g((unsigned)grid), b(GROUP * GROUPS);
+    switch (a.volt ? -1 : a.log2_nint) {  // n_int = 4, 8, 16 (the 32/16 MHz and Tiny configs) are specialised
+        case 2: fused_pair_kernel<N, 2><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        case 3: fused_pair_kernel<N, 3><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        case 4: fused_pair_kernel<N, 4><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        default: fused_pair_kernel<N, -1><<<g, b, smem_bytes<N>(), st>>>(a); break;
+    }
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;
 }
