@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--duration", type=float, default=0.0, help="override the workload's seconds of data (debug)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT+elementwise reference point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the cpu_baseline leg")
     return ap.parse_args()
 
@@ -172,6 +173,37 @@ def oracle_timed(w, x, n_threads: int, target_s: float):
     assert out.shape[2] == nb * (L // w.n_int)
     samples = w.n_chan * nb * L
     return samples / dt / 1e6, dt, nb, nb_all
+
+
+def cufft_chain_reference(w, plan, d_in, chirp_host, steps: int = 3):
+    """REFERENCE POINT ONLY (BASELINE.json north_star: "cuFFT+elementwise is timed only as a reference point"): the same
+    framing computed as an unfused chain of library calls -- unpack, torch.fft.fft (cuFFT), chirp multiply,
+    torch.fft.ifft, slice, abs^2, integrate -- each a full HBM round trip.  Nothing of this is in the product."""
+    import torch
+    N, L, head, n_int = plan.n_fft, plan.L, plan.head, plan.n_int
+    T = d_in.shape[0]
+    nb = plan.n_blocks(T)
+    h = torch.from_numpy(chirp_host).cuda().to(torch.complex64)          # [C][N], includes 1/N; norm="forward" undoes it
+
+    def chain():
+        x = torch.view_as_complex(d_in.permute(1, 0, 2).to(torch.float32).contiguous())      # [C][T]
+        blocks = x[:, : (nb - 1) * L + N].unfold(1, N, L)                                     # [C][nb][N] view
+        spec = torch.fft.fft(blocks, dim=-1)
+        spec *= h[:, None, :] * N
+        v = torch.fft.ifft(spec, dim=-1)[:, :, head:head + L]
+        p = (v.real * v.real + v.imag * v.imag).reshape(w.n_chan, nb * L // n_int, n_int).sum(-1)
+        return p
+
+    out = chain()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        out = chain()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    return out, ms
 
 
 def run_reference(args):
@@ -329,6 +361,22 @@ def run_ours(args):
                "equals_device_resident_output": same}
         del h_out
 
+    # ---- cuFFT + elementwise chain on the same framing: a reference point, never part of the product --------------------
+    cufft_ref = None
+    if not args.no_cufft and rank == 0 and plan.n_dm == 1:
+        try:
+            import numpy as np
+            chirp_host = np.stack([plan.debug_chirp(0, c) for c in range(w.n_chan)]).astype(np.complex64)
+            ref_out, ref_ms = cufft_chain_reference(w, plan, d_in, chirp_host)
+            rel = float(((ref_out - d_out[0]).norm() / d_out[0].norm()).item())
+            cufft_ref = {"ms_per_step": ref_ms, "value": samples / (ref_ms * 1e-3) / 1e6, "unit": UNIT,
+                         "speedup_of_fused_path": ref_ms / ms_step, "rel_l2_vs_fused_output": rel,
+                         "what": "torch (cuFFT) unpack -> fft -> chirp -> ifft -> slice -> abs^2 -> integrate, unfused"}
+            del ref_out
+            torch.cuda.empty_cache()
+        except Exception as exc:            # the reference point must never take the bench down
+            cufft_ref = {"error": repr(exc)[:200]}
+
     # ---- roofline of the dominant (fused) kernel --------------------------------------------------------------------
     peaks, peaks_src = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
@@ -388,7 +436,8 @@ def run_ours(args):
                          "input smaller than 2x L2: numbers include L2 hits",
                    "sharding": "one workload-sized batch per rank, no data-path collective"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps,
-        "roofline": roofline, "cpu_baseline": cpu, "checksum_mean_first_1000": checksum,
+        "roofline": roofline, "cpu_baseline": cpu, "cufft_reference_point": cufft_ref,
+        "checksum_mean_first_1000": checksum,
     }
     print(json.dumps(line), flush=True)
     plan.destroy()

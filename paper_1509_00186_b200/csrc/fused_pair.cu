@@ -124,7 +124,11 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
     };
 
     int cur_chan = -1;
-    if (s_begin < s_end) prefetch(s_begin);
+    if (s_begin < s_end) {
+        prefetch(s_begin);
+        cp_async_wait_all();
+        group_bar(bar_id, GROUP);
+    }
 
     for (int s = s_begin; s < s_end; ++s) {
         const int c = s / a.spc;
@@ -139,8 +143,7 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
             cur_chan = c;
             __syncthreads();
         }
-        cp_async_wait_all();
-        group_bar(bar_id, GROUP);
+        // (the staged rows of this super-item are complete and visible: see the barrier that ends the previous one)
 
         // 1b. unpack int8 (re, im) -> fp32, exact: bytes -> 0x4B0000uu (= 2^23 + u, u = x + 128) -> minus (2^23 + 128)
         C2 x[16];
@@ -203,6 +206,7 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
                                                                  : make_float2(x[m].re.x, x[m].im.x);
                     }
                 }
+                cp_async_wait_all();
                 group_bar(bar_id, GROUP);
                 continue;
             }
@@ -244,7 +248,10 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
                     if (liveB) dstB[o] = acc.y;
                 }
             }
-            group_bar(bar_id, GROUP);  // the power cells live in the exchange buffer of the next transform
+            // one barrier for two hand-overs: the power cells live in the exchange buffer of the next transform, and the
+            // rows prefetched for the next super-item (issued during this one's first exchange) are now visible
+            cp_async_wait_all();
+            group_bar(bar_id, GROUP);
         }
     }
 }
