@@ -39,7 +39,7 @@ N_SM, FP32_LANES_PER_SM = 148, 128   # B200: 148 SMs x 4 sub-partitions x 32 FP3
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full`
 # capture (profiles/), keyed by workload; None until a capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"gmrt32": 1.050e9 + 0.485e9}   # profiles/r1a_ncu_gmrt32.md
+NCU_TRAFFIC_BYTES = {"gmrt32": 1.0417e9 + 0.4829e9}   # profiles/r1f_ncu_gmrt32.md
 
 
 def parse_args():
