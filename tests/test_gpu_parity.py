@@ -168,6 +168,35 @@ def test_small_cases_full_parity(dd, torch, n_fft, n_int, dm, n_chan, taper):
         assert_parity(got, ref, L // n_int)
 
 
+@pytest.mark.parametrize("n_fft,n_int,dm,n_chan,n_blocks", [
+    (4096, 256, (5.0,), 3, 4),          # n_int > 128: the pair kernel's epilogue sums more than 4 samples per lane
+    (1024, 512, (0.5,), 9, 5),          # one output per block and channel
+    (2048, 1, (20.0,), 2, 2),           # no integration at all
+    (4096, 4, (71.0,), 1, 1),           # a single (channel, block) unit: one half-empty pair
+    (1024, 16, (10.0,), 1, 17),         # one channel, an odd number of blocks, several super-items
+    (16384, 1, (100.0,), 1, 1),
+])
+def test_degenerate_shapes_full_parity(dd, torch, n_fft, n_int, dm, n_chan, n_blocks):
+    bw = 62.5e3 * n_chan
+    cfg = oracle.OracleConfig(n_chan, bw, 325e6 if n_fft < 16384 else 150e6, dm, n_fft, n_int)
+    head, tail, L = oracle.framing(cfg)
+    n_samp = n_blocks * L + head + tail          # exactly n_blocks blocks, no tail
+    x = datagen.noise_only(n_samp, n_chan, seed=3 * n_fft + n_int)
+    ref = oracle.dedisp(cfg, x, n_threads=NT)
+    with dd.dedisp_plan(n_chan, bw, cfg.f_center_hz, dm, n_fft, n_int) as plan:
+        assert plan.n_blocks(n_samp) == n_blocks and plan.n_blocks(n_samp - 1) == n_blocks - 1
+        got = run_gpu(torch, plan, x)
+        assert_parity(got, ref, L // n_int)
+        if n_blocks > 1:                         # one sample short of the last block: that block must not be written
+            out = torch.full((len(dm), n_chan, got.shape[2]), -1.0, dtype=torch.float32, device="cuda")
+            plan.execute(torch.from_numpy(x[:-1]).cuda(), out)
+            torch.cuda.synchronize()
+            o = out.cpu().numpy()
+            per = L // n_int
+            assert np.array_equal(o[:, :, : (n_blocks - 1) * per], got[:, :, : (n_blocks - 1) * per])
+            assert (o[:, :, (n_blocks - 1) * per:] == -1.0).all()
+
+
 def test_voltage_hook_matches_oracle_voltages(dd, torch):
     w = datagen.WORKLOADS["gmrt32"].scaled(0.2)
     chans = [0, 255, 511]
