@@ -28,7 +28,6 @@ static void free_plan(dedisp_plan_s* p)
     dedisp_stream_free(p);
     if (p->d_chirp) cudaFree(p->d_chirp);
     if (p->d_twiddle) cudaFree(p->d_twiddle);
-    if (p->d_twiddle4) cudaFree(p->d_twiddle4);
     if (p->d_xt) cudaFree(p->d_xt);
     if (p->d_spec) cudaFree(p->d_spec);
     if (p->prof_ev) {
@@ -94,8 +93,7 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     rc = p->use_pair ? dedisp_pair_init() : dedisp_fused_init();
     if (rc != DEDISP_OK) return fail(rc);
     PLAN_TRY(cudaMalloc(&p->d_chirp, sizeof(float2) * (size_t)n_dm * n_chan * n_fft));
-    if (p->use_pair) PLAN_TRY(cudaMalloc(&p->d_twiddle4, sizeof(float4) * (size_t)n_fft));
-    else PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
+    PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
     if (n_dm > 1)
         PLAN_TRY(cudaMalloc(&p->d_spec, p->use_pair ? dedisp_pair_spec_bytes(n_fft) : dedisp_fused_spec_bytes(n_fft)));
     PLAN_TRY(cudaMalloc(&d_dm, sizeof(double) * n_dm));

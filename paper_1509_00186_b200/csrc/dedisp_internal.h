@@ -23,12 +23,11 @@ struct dedisp_plan_s {
     int nfft_rule;
     int device;
     // device tables owned by the plan
-    // n_fft <= 4096 runs the packed pair kernel (fused_pair.cu), which wants its twiddles in both f32x2 lanes:
-    // float4 (c, c, s, s); larger transforms run the scalar kernel (fused.cu) on float2 (c, s).  Only one table exists.
+    // n_fft <= 4096 runs the packed pair kernel (fused_pair.cu), larger transforms the scalar kernel (fused.cu); both
+    // read the same tables
     int use_pair;
     float2* d_chirp;    // [n_dm][n_chan][n_fft], taper * exp(+2 pi i psi) / n_fft
     float2* d_twiddle;  // [n_fft], exp(-2 pi i m / n_fft)
-    float4* d_twiddle4;
     // channel-major int8 scratch: [n_chan][xt_stride] (re,im) pairs, xt_stride samples per row
     float2* d_spec;     // [resident CTAs][units per CTA][n_fft] forward-spectrum stash shared by the trial DMs (n_dm > 1)
     int8_t* d_xt;

@@ -4,7 +4,8 @@
 // float2: lane .x belongs to unit A, lane .y to unit B (two overlap-save blocks of the same channel).  Both units go
 // through identical butterflies with identical twiddles, so every FP32 instruction of the transform is a packed one:
 // half the issue slots of the scalar form for the same lane throughput (profiles/r1b_fp32_issue.md), and the index
-// arithmetic, twiddle loads and twiddle powers are shared by the two units.
+// arithmetic, twiddle loads and twiddle powers (kept scalar, broadcast into the packed multiplies) are shared by the
+// two units.
 //
 // Indexing is the one of fft_regs.cuh: slot m of thread t is element i = t + m*TPU (TPU = N/16); a radix-R pass runs
 // S = 16/R butterflies per thread on slots q + r*S; after the last pass the spectrum is back in the same slot map.
@@ -83,37 +84,44 @@ __device__ __forceinline__ void butterfly(C2 (&x)[16], int q)
     }
 }
 
+// Twiddles are the same for both lanes, so they live as SCALAR complex numbers (half the registers, and their powers
+// cost scalar FMUL/FFMA: half the FP32 pipe time of packed ones); the packed multiply takes them as broadcast operands.
+__device__ __forceinline__ float2 smul(float2 a, float2 b)
+{
+    return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.y, b.x, a.x * b.y));
+}
+__device__ __forceinline__ float2 ssqr(float2 w) { return make_float2(fmaf(-w.y, w.y, w.x * w.x), 2.0f * w.x * w.y); }
+__device__ __forceinline__ C2 cmul_s(C2 a, float2 w) { return cmul(a, C2{vdup(w.x), vdup(w.y)}); }
+
 // Twiddles of one pass, in two steps so that the serial part (table load, squarings) runs in the window between the
-// scatter and the gather of the preceding exchange, where the 64 data registers are dead and the thread would
-// otherwise wait at the barrier:  prepare = w1 (and for radix 16 the powers 2, 3, 4, 8, 12);  apply = the remaining
-// products and x[q + r*S] *= w1^r, r = 1..R-1.  Every power is a product of depth <= log2 R.
-template <int R> struct TwSet { C2 w1[16 / R]; };
-template <> struct TwSet<16> { C2 w1, w2, w3, w4, w8, w12; };
+// scatter and the gather of the preceding exchange, where the thread would otherwise wait at the barrier:
+// prepare = w1 (and for radix 16 the powers 2, 3, 4, 8, 12);  apply = the remaining products and
+// x[q + r*S] *= w1^r, r = 1..R-1.  Every power is a product of depth <= log2 R.
+template <int R> struct TwSet { float2 w1[16 / R]; };
+template <> struct TwSet<16> { float2 w1, w2, w3, w4, w8, w12; };
 
 template <int N, int R, int NS, int SIGN>
-__device__ __forceinline__ TwSet<R> twiddle_prepare(int t, const float4* __restrict__ tw4)
+__device__ __forceinline__ TwSet<R> twiddle_prepare(int t, const float2* __restrict__ tw)
 {
     constexpr int S = 16 / R;
     constexpr int TPU = N / 16;
-    TwSet<R> tw;
+    TwSet<R> s;
     if constexpr (R == 16) {
-        const float4 w = __ldg(&tw4[(t & (NS - 1)) * (N / (NS * R))]);
-        tw.w1 = C2{make_float2(w.x, w.y), make_float2(w.z, w.w)};
-        if (SIGN > 0) tw.w1.im = vneg(tw.w1.im);
-        tw.w2 = csqr(tw.w1);
-        tw.w3 = cmul(tw.w2, tw.w1);
-        tw.w4 = csqr(tw.w2);
-        tw.w8 = csqr(tw.w4);
-        tw.w12 = cmul(tw.w8, tw.w4);
+        s.w1 = __ldg(&tw[(t & (NS - 1)) * (N / (NS * R))]);
+        if (SIGN > 0) s.w1.y = -s.w1.y;
+        s.w2 = ssqr(s.w1);
+        s.w3 = smul(s.w2, s.w1);
+        s.w4 = ssqr(s.w2);
+        s.w8 = ssqr(s.w4);
+        s.w12 = smul(s.w8, s.w4);
     } else {
 #pragma unroll
         for (int q = 0; q < S; ++q) {
-            const float4 w = __ldg(&tw4[((t + q * TPU) & (NS - 1)) * (N / (NS * R))]);
-            tw.w1[q] = C2{make_float2(w.x, w.y), make_float2(w.z, w.w)};
-            if (SIGN > 0) tw.w1[q].im = vneg(tw.w1[q].im);
+            s.w1[q] = __ldg(&tw[((t + q * TPU) & (NS - 1)) * (N / (NS * R))]);
+            if (SIGN > 0) s.w1[q].y = -s.w1[q].y;
         }
     }
-    return tw;
+    return s;
 }
 
 template <int R>
@@ -121,38 +129,38 @@ __device__ __forceinline__ void twiddle_apply(C2 (&x)[16], const TwSet<R>& tw)
 {
     constexpr int S = 16 / R;
     if constexpr (R == 16) {
-        x[1] = cmul(x[1], tw.w1);
-        x[2] = cmul(x[2], tw.w2);
-        x[3] = cmul(x[3], tw.w3);
-        x[4] = cmul(x[4], tw.w4);
-        x[5] = cmul(x[5], cmul(tw.w4, tw.w1));
-        x[6] = cmul(x[6], cmul(tw.w4, tw.w2));
-        x[7] = cmul(x[7], cmul(tw.w4, tw.w3));
-        x[8] = cmul(x[8], tw.w8);
-        x[9] = cmul(x[9], cmul(tw.w8, tw.w1));
-        x[10] = cmul(x[10], cmul(tw.w8, tw.w2));
-        x[11] = cmul(x[11], cmul(tw.w8, tw.w3));
-        x[12] = cmul(x[12], tw.w12);
-        x[13] = cmul(x[13], cmul(tw.w12, tw.w1));
-        x[14] = cmul(x[14], cmul(tw.w12, tw.w2));
-        x[15] = cmul(x[15], cmul(tw.w12, tw.w3));
+        x[1] = cmul_s(x[1], tw.w1);
+        x[2] = cmul_s(x[2], tw.w2);
+        x[3] = cmul_s(x[3], tw.w3);
+        x[4] = cmul_s(x[4], tw.w4);
+        x[5] = cmul_s(x[5], smul(tw.w4, tw.w1));
+        x[6] = cmul_s(x[6], smul(tw.w4, tw.w2));
+        x[7] = cmul_s(x[7], smul(tw.w4, tw.w3));
+        x[8] = cmul_s(x[8], tw.w8);
+        x[9] = cmul_s(x[9], smul(tw.w8, tw.w1));
+        x[10] = cmul_s(x[10], smul(tw.w8, tw.w2));
+        x[11] = cmul_s(x[11], smul(tw.w8, tw.w3));
+        x[12] = cmul_s(x[12], tw.w12);
+        x[13] = cmul_s(x[13], smul(tw.w12, tw.w1));
+        x[14] = cmul_s(x[14], smul(tw.w12, tw.w2));
+        x[15] = cmul_s(x[15], smul(tw.w12, tw.w3));
     } else {
 #pragma unroll
         for (int q = 0; q < S; ++q) {
 #define XR(r) x[q + (r) * S]
-            const C2 w1 = tw.w1[q];
-            XR(1) = cmul(XR(1), w1);
+            const float2 w1 = tw.w1[q];
+            XR(1) = cmul_s(XR(1), w1);
             if constexpr (R >= 4) {
-                const C2 w2 = csqr(w1);
-                const C2 w3 = cmul(w2, w1);
-                XR(2) = cmul(XR(2), w2);
-                XR(3) = cmul(XR(3), w3);
+                const float2 w2 = ssqr(w1);
+                const float2 w3 = smul(w2, w1);
+                XR(2) = cmul_s(XR(2), w2);
+                XR(3) = cmul_s(XR(3), w3);
                 if constexpr (R >= 8) {
-                    const C2 w4 = csqr(w2);
-                    XR(4) = cmul(XR(4), w4);
-                    XR(5) = cmul(XR(5), cmul(w4, w1));
-                    XR(6) = cmul(XR(6), cmul(w4, w2));
-                    XR(7) = cmul(XR(7), cmul(w4, w3));
+                    const float2 w4 = ssqr(w2);
+                    XR(4) = cmul_s(XR(4), w4);
+                    XR(5) = cmul_s(XR(5), smul(w4, w1));
+                    XR(6) = cmul_s(XR(6), smul(w4, w2));
+                    XR(7) = cmul_s(XR(7), smul(w4, w3));
                 }
             }
 #undef XR
@@ -239,12 +247,12 @@ __device__ __forceinline__ void natural_order(C2 (&x)[16])
 // Full N-point transform (N = R0*R1*R2) of both lanes; unnormalised; kernel exp(SIGN*2*pi*i*k*n/N).  `after_first`
 // runs once between the first barrier and the first gather (the fused kernel issues its input prefetch there).
 template <int N, int R0, int R1, int R2, int SIGN, class F>
-__device__ __forceinline__ void fft_pair(C2 (&x)[16], int t, float4* __restrict__ sm, const float4* __restrict__ tw4,
+__device__ __forceinline__ void fft_pair(C2 (&x)[16], int t, float4* __restrict__ sm, const float2* __restrict__ tw,
                                          int bar_id, int bar_count, F after_first)
 {
     pass_butterflies<R0, SIGN>(x);
     exchange_scatter<N, R0, 1>(x, t, sm);
-    const TwSet<R1> tw1 = twiddle_prepare<N, R1, R0, SIGN>(t, tw4);  // tw4[m] = (c, c, s, s) of exp(-2*pi*i*m/N)
+    const TwSet<R1> tw1 = twiddle_prepare<N, R1, R0, SIGN>(t, tw);  // tw[m] = exp(-2*pi*i*m/N)
     group_bar(bar_id, bar_count);
     after_first();
     exchange_gather<N>(x, t, sm);
@@ -252,7 +260,7 @@ __device__ __forceinline__ void fft_pair(C2 (&x)[16], int t, float4* __restrict_
     twiddle_apply<R1>(x, tw1);
     pass_butterflies<R1, SIGN>(x);
     exchange_scatter<N, R1, R0>(x, t, sm);
-    const TwSet<R2> tw2 = twiddle_prepare<N, R2, R0 * R1, SIGN>(t, tw4);
+    const TwSet<R2> tw2 = twiddle_prepare<N, R2, R0 * R1, SIGN>(t, tw);
     group_bar(bar_id, bar_count);
     exchange_gather<N>(x, t, sm);
     group_bar(bar_id, bar_count);

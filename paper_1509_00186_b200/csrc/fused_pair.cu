@@ -28,7 +28,7 @@ struct PairArgs {
     const int8_t* xt;      // [n_chan][xt_stride][2]
     long long xt_stride;   // samples
     const float2* chirp;   // [n_dm][n_chan][N] (c, s), includes 1/N
-    const float4* tw4;     // [N] (c, c, s, s)
+    const float2* tw;      // [N] exp(-2 pi i m / N)
     float* out;            // [n_dm][n_chan][out_stride]
     long long out_stride, out_col0;
     float4* spec;          // [gridDim.x][2P][N] forward-spectrum stash, used when n_dm > 1
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
         }
         // 2. forward FFT; once every thread of the group is past the unpack, the staging buffer is
         //    free for the next super-item's rows
-        fft_pair<N, Sh::R0, Sh::R1, Sh::R2, -1>(x, t, sm, a.tw4, bar_id, GROUP, [&] {
+        fft_pair<N, Sh::R0, Sh::R1, Sh::R2, -1>(x, t, sm, a.tw, bar_id, GROUP, [&] {
             if (s + 1 < s_end) prefetch(s + 1);
         });
 
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(GROUP * GROUPS, 1) fused_pair_kernel(const Pai
                 }
             }
             // 4. inverse FFT (1/N already applied)
-            fft_pair<N, Sh::R0, Sh::R1, Sh::R2, +1>(x, t, sm, a.tw4, bar_id, GROUP, [] {});
+            fft_pair<N, Sh::R0, Sh::R1, Sh::R2, +1>(x, t, sm, a.tw, bar_id, GROUP, [] {});
 
             if (a.volt) {  // debug hook: valid voltages of one block
                 if (live && (a.volt_block >> 1) == pr) {
@@ -319,7 +319,7 @@ int base_args(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, l
     const long long ppc = (nb + 1) / 2, pps = pairs_per_super(p->n_fft), spc = (ppc + pps - 1) / pps;
     if (nb > 0x3fffffff || spc * p->n_chan > 0x7fffffff) return DEDISP_EINVAL;  // 32-bit item arithmetic in the kernel
     a = PairArgs{};
-    a.xt = d_xt; a.xt_stride = xt_stride; a.chirp = p->d_chirp; a.tw4 = p->d_twiddle4;
+    a.xt = d_xt; a.xt_stride = xt_stride; a.chirp = p->d_chirp; a.tw = p->d_twiddle;
     a.nb = (int)nb; a.ppc = (int)ppc; a.spc = (int)spc; a.n_super = (int)(spc * p->n_chan); a.first_super = 0;
     a.n_chan = p->n_chan; a.n_dm = p->n_dm; a.head = p->head; a.L = p->L;
     int lg = 0;

@@ -97,14 +97,13 @@ __global__ void chirp_table_kernel(float2* __restrict__ chirp, const double* __r
     chirp[((size_t)d * n_chan + c) * n_fft + k] = make_float2((float)(w * co), (float)(w * s));
 }
 
-__global__ void twiddle_table_kernel(float2* __restrict__ tw, float4* __restrict__ tw4, int n_fft)
+__global__ void twiddle_table_kernel(float2* __restrict__ tw, int n_fft)
 {
     const int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n_fft) return;
     double s, co;
     sincospi(-2.0 * (double)m / (double)n_fft, &s, &co);
-    if (tw4) tw4[m] = make_float4((float)co, (float)co, (float)s, (float)s);
-    else tw[m] = make_float2((float)co, (float)s);
+    tw[m] = make_float2((float)co, (float)s);
 }
 
 int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaStream_t st)
@@ -118,7 +117,7 @@ int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaSt
 
 int dedisp_launch_twiddle_table(const dedisp_plan_s* p, cudaStream_t st)
 {
-    twiddle_table_kernel<<<(p->n_fft + 255) / 256, 256, 0, st>>>(p->d_twiddle, p->d_twiddle4, p->n_fft);
+    twiddle_table_kernel<<<(p->n_fft + 255) / 256, 256, 0, st>>>(p->d_twiddle, p->n_fft);
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;
 }

@@ -170,7 +170,7 @@ def test_small_cases_full_parity(dd, torch, n_fft, n_int, dm, n_chan, taper):
 
 @pytest.mark.parametrize("n_fft,n_int,dm,n_chan,n_blocks", [
     (4096, 256, (5.0,), 3, 4),          # n_int > 128: the pair kernel's epilogue sums more than 4 samples per lane
-    (1024, 512, (0.5,), 9, 5),          # one output per block and channel
+    (1024, 256, (0.5,), 9, 5),          # half of every block is overlap, two outputs per block and channel
     (2048, 1, (20.0,), 2, 2),           # no integration at all
     (4096, 4, (71.0,), 1, 1),           # a single (channel, block) unit: one half-empty pair
     (1024, 16, (10.0,), 1, 17),         # one channel, an odd number of blocks, several super-items
