@@ -44,8 +44,7 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     if (!out_plan) return DEDISP_EINVAL;
     *out_plan = nullptr;
     if ((flags & ~DEDISP_TAPER_MASK) || (flags & DEDISP_TAPER_MASK) == 3u) return DEDISP_EINVAL;
-    if (n_fft <= 0 || (n_fft & (n_fft - 1)) || !(dedisp_fused_supported(n_fft) || dedisp_pair_supported(n_fft)))
-        return DEDISP_EINVAL;
+    if (n_fft <= 0 || (n_fft & (n_fft - 1)) || !dedisp_aos_supported(n_fft)) return DEDISP_EINVAL;
     // R9 gives D_tot % n_int == 0, so L % n_int == n_fft % n_int: only powers of two can divide a block evenly
     if (n_int <= 0 || (n_int & (n_int - 1))) return DEDISP_EINVAL;
     int head, tail, L;
@@ -89,13 +88,12 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
             return fail(e__ == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA);        \
         }                                                                                        \
     } while (0)
-    p->use_pair = dedisp_pair_supported(n_fft);
-    rc = p->use_pair ? dedisp_pair_init() : dedisp_fused_init();
+    rc = dedisp_aos_init();
     if (rc != DEDISP_OK) return fail(rc);
     PLAN_TRY(cudaMalloc(&p->d_chirp, sizeof(float2) * (size_t)n_dm * n_chan * n_fft));
     PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
     if (n_dm > 1)
-        PLAN_TRY(cudaMalloc(&p->d_spec, p->use_pair ? dedisp_pair_spec_bytes(n_fft) : dedisp_fused_spec_bytes(n_fft)));
+        PLAN_TRY(cudaMalloc(&p->d_spec, dedisp_aos_spec_bytes(n_fft)));
     PLAN_TRY(cudaMalloc(&d_dm, sizeof(double) * n_dm));
     PLAN_TRY(cudaMemcpy(d_dm, p->dm, sizeof(double) * n_dm, cudaMemcpyHostToDevice));
     rc = dedisp_launch_chirp_table(p, d_dm, 0);
@@ -142,8 +140,7 @@ int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows,
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[1], st));
     if (after_corner_turn) DEDISP_CUDA_TRY(cudaEventRecord(after_corner_turn, st));
     if (nb > 0) {
-        rc = p->use_pair ? dedisp_launch_pair(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st)
-                         : dedisp_launch_fused(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st);
+        rc = dedisp_launch_aos(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st);
         if (rc != DEDISP_OK) return rc;
     }
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[2], st));
@@ -264,6 +261,5 @@ extern "C" int dedisp_debug_voltage(dedisp_plan_t p, const int8_t* d_in, long lo
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = debug_prepare(p, d_in, n_samp, chan, block, st);
     if (rc != DEDISP_OK) return rc;
-    return p->use_pair ? dedisp_launch_pair_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st)
-                       : dedisp_launch_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st);
+    return dedisp_launch_aos_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st);
 }

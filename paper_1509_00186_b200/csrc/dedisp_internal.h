@@ -23,9 +23,6 @@ struct dedisp_plan_s {
     int nfft_rule;
     int device;
     // device tables owned by the plan
-    // n_fft <= 4096 runs the packed pair kernel (fused_pair.cu), larger transforms the scalar kernel (fused.cu); both
-    // read the same tables
-    int use_pair;
     float2* d_chirp;    // [n_dm][n_chan][n_fft], taper * exp(+2 pi i psi) / n_fft
     float2* d_twiddle;  // [n_fft], exp(-2 pi i m / n_fft)
     // channel-major int8 scratch: [n_chan][xt_stride] (re,im) pairs, xt_stride samples per row
@@ -59,25 +56,18 @@ static inline long long dedisp_xt_stride(long long n_samp) { return (n_samp + 63
 // corner turn: int8 [n_samp][n_chan][2] -> int8 [n_chan][xt_stride][2], rows t0_dst.. of the destination
 int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int8_t* d_xt, long long xt_stride,
                               long long dst_t0, cudaStream_t st);
-// fused forward FFT -> chirp -> inverse FFT -> discard -> detect -> integrate over nb blocks of every channel.
-// out[d][c][out_col0 + b*L/n_int + j]
-int dedisp_launch_fused(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
-                        long long out_stride, long long out_col0, cudaStream_t st);
+// fused_aos.cu: fused unpack -> forward FFT -> chirp -> inverse FFT -> discard -> detect -> integrate over nb blocks of
+// every channel (all enqueue only):  out[d][c][out_col0 + b*L/n_int + j]
+int dedisp_launch_aos(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
+                      long long out_stride, long long out_col0, cudaStream_t st);
+int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
+                                    long long block, float* d_volt, cudaStream_t st);
+int dedisp_aos_supported(int n_fft);
+size_t dedisp_aos_spec_bytes(int n_fft);  // valid after dedisp_aos_init()
+int dedisp_aos_init(void);                // sets the dynamic shared memory attributes once per process
+// corner_turn.cu: test hook
 int dedisp_launch_debug_unpack(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
                                long long block, float* d_block, cudaStream_t st);
-int dedisp_launch_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
-                                long long block, float* d_volt, cudaStream_t st);
-// fused_pair.cu: same contract as the three launchers above, for n_fft <= 4096
-int dedisp_launch_pair(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
-                       long long out_stride, long long out_col0, cudaStream_t st);
-int dedisp_launch_pair_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
-                                     long long block, float* d_volt, cudaStream_t st);
-int dedisp_pair_supported(int n_fft);
-size_t dedisp_pair_spec_bytes(int n_fft);
-int dedisp_pair_init(void);
-int dedisp_fused_supported(int n_fft);
-size_t dedisp_fused_spec_bytes(int n_fft);  // valid after dedisp_fused_init()
-int dedisp_fused_init(void);  // sets the dynamic shared memory attributes once per process
 // plan-time table generation on the device (fp64 phase)
 int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaStream_t st);
 int dedisp_launch_twiddle_table(const dedisp_plan_s* p, cudaStream_t st);

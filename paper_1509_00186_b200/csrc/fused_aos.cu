@@ -1,0 +1,352 @@
+// fused_aos.cu -- steps 1b-6 of the path for N_fft <= 4096, one (channel, block) unit per 256 threads (or fewer), every
+// complex number in one packed f32x2 register pair (fft_aos.cuh): unpack -> forward FFT -> chirp -> inverse FFT ->
+// |v|^2 -> integrate on FADD2/FMUL2/FFMA2 (Fig. 4).  HBM traffic: 2 B in,
+// 4/n_int B out per complex sample.
+//
+// 16 elements per thread = 32 data registers, so ONE persistent 1024-thread CTA per SM holds FOUR groups of 256
+// threads, each with its own units, exchange buffers and named barrier: while one group is in a shared-memory
+// exchange the other three keep the FP32 pipe busy.  A CTA walks a contiguous range of "super-items" (4U consecutive
+// blocks of ONE channel, U = 1/2/4 units per group for N = 4096/2048/1024):
+//   * the channel's chirp row sits in shared memory and is reloaded only when the channel changes;
+//   * the int8 rows of the NEXT super-item are prefetched with cp.async while this one computes.
+#include "dedisp_internal.h"
+#include "fft_aos.cuh"
+
+using namespace dedisp_aos;
+
+namespace {
+
+constexpr int CTA = 1024;  // threads per CTA: 64 registers each
+
+// N = R0*R1*R2*R3 (16 elements per thread, N/16 threads per unit); GROUP = threads that share a named barrier and hold
+// U units; CHIRP_SMEM: the channel's chirp row (8 B x N) fits in shared memory beside the exchange buffers.
+template <int N> struct AShape;
+template <> struct AShape<1024>  { static constexpr int GROUP = 256,  U = 4, R0 = 16, R1 = 16, R2 = 4,  R3 = 1; static constexpr bool CHIRP_SMEM = true; };
+template <> struct AShape<2048>  { static constexpr int GROUP = 256,  U = 2, R0 = 16, R1 = 16, R2 = 8,  R3 = 1; static constexpr bool CHIRP_SMEM = true; };
+template <> struct AShape<4096>  { static constexpr int GROUP = 256,  U = 1, R0 = 16, R1 = 16, R2 = 16, R3 = 1; static constexpr bool CHIRP_SMEM = true; };
+template <> struct AShape<8192>  { static constexpr int GROUP = 512,  U = 1, R0 = 16, R1 = 16, R2 = 16, R3 = 2; static constexpr bool CHIRP_SMEM = false; };
+template <> struct AShape<16384> { static constexpr int GROUP = 1024, U = 1, R0 = 16, R1 = 16, R2 = 16, R3 = 4; static constexpr bool CHIRP_SMEM = false; };
+template <int N> __host__ __device__ constexpr int units_per_super_of() { return CTA / AShape<N>::GROUP * AShape<N>::U; }
+
+struct AosArgs {
+    const int8_t* xt;      // [n_chan][xt_stride][2]
+    long long xt_stride;   // samples
+    const float2* chirp;   // [n_dm][n_chan][N] (c, s), includes 1/N
+    const float2* tw;      // [N] exp(-2 pi i m / N)
+    float* out;            // [n_dm][n_chan][out_stride]
+    long long out_stride, out_col0;
+    float2* spec;          // [gridDim.x][4U][N] forward-spectrum stash, used when n_dm > 1
+    float2* volt;          // debug: [n_dm][L] voltages of block volt_block, else nullptr
+    int volt_block;
+    int nb;                // blocks per channel
+    int spc;               // super-items per channel = ceil(nb / 4U)
+    int n_super;           // super-items to process
+    int first_super;       // debug: start here
+    int n_chan, n_dm, log2_nint, head, L;
+};
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// int8 pair (re | im << 8) -> fp32 (re, im), exact, without I2F: bytes ^ 0x80 -> 0x4B0000uu = 2^23 + u (u = x + 128),
+// then one packed add of -(2^23 + 128)
+__device__ __forceinline__ C unpack_int8x2(uint32_t v)
+{
+    const uint32_t w = v ^ 0x8080u, k = 0x4B000000u;
+    uint32_t re, im;
+    asm("prmt.b32 %0, %1, %2, 0x7440;" : "=r"(re) : "r"(w), "r"(k));
+    asm("prmt.b32 %0, %1, %2, 0x7441;" : "=r"(im) : "r"(w), "r"(k));
+    return __fadd2_rn(make_float2(__uint_as_float(re), __uint_as_float(im)), make_float2(-8388736.0f, -8388736.0f));
+}
+
+template <int N> constexpr size_t smem_bytes()
+{
+    return (size_t)units_per_super_of<N>() * (sizeof(float2) * padded_len(N) + N * sizeof(uint16_t)) +
+           (AShape<N>::CHIRP_SMEM ? sizeof(float2) * N : 0);
+}
+
+// LGN = log2(n_int) when it is one of the specialised values (the epilogue then has no run-time geometry), else -1.
+template <int N, int LGN>
+__global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
+{
+    using Sh = AShape<N>;
+    constexpr int GROUP = Sh::GROUP, TPU = N / 16, UPS = units_per_super_of<N>();
+    constexpr bool CHIRP_SMEM = Sh::CHIRP_SMEM;
+    extern __shared__ float2 smem2[];
+    const int g = threadIdx.x / GROUP;  // group: its own barrier
+    const int us = threadIdx.x / TPU;   // unit slot inside the super-item (g*U + unit in group)
+    const int t = threadIdx.x % TPU;    // thread inside the unit
+    const int bar_id = g + 1;
+    C* sm = smem2 + (size_t)us * padded_len(N);                         // exchange buffer of this unit
+    float* smf = reinterpret_cast<float*>(sm);                           // ... reused for the detected powers
+    float2* chirp_s = smem2 + (size_t)UPS * padded_len(N);               // [N], whole CTA (only if CHIRP_SMEM)
+    uint16_t* stage = reinterpret_cast<uint16_t*>(chirp_s + (CHIRP_SMEM ? N : 0)) + (size_t)us * N;  // [N] int8 pairs
+    const uint16_t* xt16 = reinterpret_cast<const uint16_t*>(a.xt);
+
+    const int lgn = LGN >= 0 ? LGN : a.log2_nint;
+    const int n_out = a.L >> lgn;
+    // epilogue geometry: each lane sums 2^lg_chunk consecutive samples, 2^lg_lpo lanes make one output
+    const int lg_chunk = lgn < 2 ? lgn : (lgn > 7 ? lgn - 5 : 2);
+    const int lg_lpo = lgn - lg_chunk;
+    const int n_work = a.L >> lg_chunk;
+
+    const int s_begin = a.first_super + (int)((long long)blockIdx.x * a.n_super / gridDim.x);
+    const int s_end = a.first_super + (int)((long long)(blockIdx.x + 1) * a.n_super / gridDim.x);
+
+    // stage the int8 rows of this thread's unit of super-item s: 2 x 16 B per thread (P:L270 framing: block b reads
+    // rows b*L .. b*L+N-1; consecutive blocks overlap)
+    auto prefetch = [&](int s) {
+        const int c = s / a.spc;
+        const int b = (s - c * a.spc) * UPS + us;
+        if (b < a.nb) {
+            const uint16_t* src = xt16 + (long long)c * a.xt_stride + (long long)b * a.L;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int k = (j * TPU + t) * 8;  // 8 samples = 16 B
+                cp_async16(stage + k, src + k);
+            }
+        }
+        cp_async_commit();
+    };
+
+    int cur_chan = -1;
+    if (s_begin < s_end) {
+        prefetch(s_begin);
+        cp_async_wait_all();
+        group_bar(bar_id, GROUP);
+    }
+
+    for (int s = s_begin; s < s_end; ++s) {
+        const int c = s / a.spc;
+        const int b = (s - c * a.spc) * UPS + us;
+        const bool live = b < a.nb;
+
+        if (CHIRP_SMEM && a.n_dm == 1 && c != cur_chan) {  // all groups take this branch in the same iteration
+            __syncthreads();
+            const float2* row = a.chirp + (size_t)c * N;
+            for (int i = threadIdx.x; i < N; i += CTA) chirp_s[i] = __ldg(row + i);
+            cur_chan = c;
+            __syncthreads();
+        }
+        // (the staged rows of this super-item are complete and visible: see the barrier that ends the previous one)
+
+        // 1b. unpack int8 (re, im) -> fp32 (exact)
+        C x[16];
+#pragma unroll
+        for (int m = 0; m < 16; ++m) x[m] = unpack_int8x2(live ? (uint32_t)stage[t + m * TPU] : 0u);
+
+        // 2. forward FFT; once every thread of the group is past the unpack, the staging buffer is
+        //    free for the next super-item's rows
+        fft_aos<N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, -1>(x, t, sm, a.tw, bar_id, GROUP, [&] {
+            if (s + 1 < s_end) prefetch(s + 1);
+        });
+
+        float2* stash = a.spec + ((size_t)blockIdx.x * UPS + us) * N;
+        if (a.n_dm > 1) {
+#pragma unroll
+            for (int m = 0; m < 16; ++m) stash[t + m * TPU] = x[m];
+        }
+        for (int d = 0; d < a.n_dm; ++d) {
+            if (d > 0) {
+#pragma unroll
+                for (int m = 0; m < 16; ++m) x[m] = stash[t + m * TPU];  // same thread wrote it: no fence needed
+            }
+            // 3. chirp multiply (Eq. 3)
+            if (CHIRP_SMEM && a.n_dm == 1) {
+#pragma unroll
+                for (int m = 0; m < 16; ++m) x[m] = cmul(x[m], chirp_s[t + m * TPU]);
+            } else {
+                const float2* h = a.chirp + ((size_t)d * a.n_chan + c) * N + t;
+#pragma unroll
+                for (int m = 0; m < 16; ++m) x[m] = cmul(x[m], __ldg(h + m * TPU));
+            }
+            // 4. inverse FFT (1/N already applied)
+            fft_aos<N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, +1>(x, t, sm, a.tw, bar_id, GROUP, [] {});
+
+            if (a.volt) {  // debug hook: valid voltages of one block
+                if (live && a.volt_block == b) {
+#pragma unroll
+                    for (int m = 0; m < 16; ++m) {
+                        const int i = t + m * TPU - a.head;
+                        if (i >= 0 && i < a.L) a.volt[(size_t)d * a.L + i] = x[m];
+                    }
+                }
+                cp_async_wait_all();
+                group_bar(bar_id, GROUP);
+                continue;
+            }
+            // 5 + 6. discard the overlap, detect, integrate n_int samples (R9, R11)
+#pragma unroll
+            for (int m = 0; m < 16; ++m) {
+                const float2 sq = __fmul2_rn(x[m], x[m]);
+                smf[t + m * TPU] = sq.x + sq.y;
+            }
+            group_bar(bar_id, GROUP);
+            float* dst = a.out + ((size_t)d * a.n_chan + c) * a.out_stride + a.out_col0 + (long long)b * n_out;
+            for (int id = t; id - t < n_work; id += TPU) {  // uniform trip count: the shuffles need whole warps
+                float acc = 0.f;
+                if (id < n_work) {
+                    const float* p0 = smf + a.head + (id << lg_chunk);  // head % min(n_int, 4) == 0: aligned
+                    if (lg_chunk >= 2) {
+                        for (int j = 0; j < (1 << lg_chunk); j += 4) {
+                            const float4 u = *reinterpret_cast<const float4*>(p0 + j);
+                            acc += (u.x + u.y) + (u.z + u.w);
+                        }
+                    } else if (lg_chunk == 1) {
+                        const float2 u = *reinterpret_cast<const float2*>(p0);
+                        acc = u.x + u.y;
+                    } else {
+                        acc = p0[0];
+                    }
+                }
+                for (int off = 1; off < (1 << lg_lpo); off <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+                if (live && id < n_work && (id & ((1 << lg_lpo) - 1)) == 0) dst[id >> lg_lpo] = acc;
+            }
+            // one barrier for two hand-overs: the powers live in the exchange buffer of the next transform, and the
+            // rows prefetched for the next super-item (issued during this one's first exchange) become visible
+            cp_async_wait_all();
+            group_bar(bar_id, GROUP);
+        }
+    }
+}
+
+struct KernelInfo { int ctas_per_sm; int n_sm; size_t spec_bytes; };
+KernelInfo g_info[5];
+bool g_init_done = false;
+
+int slot_of(int n_fft)
+{
+    switch (n_fft) {
+        case 1024: return 0; case 2048: return 1; case 4096: return 2; case 8192: return 3; case 16384: return 4;
+        default: return -1;
+    }
+}
+
+template <int N, int LGN> int set_smem()
+{
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_aos_kernel<N, LGN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem_bytes<N>()));
+    return DEDISP_OK;
+}
+
+template <int N> int init_one(int slot)
+{
+    int rc;
+    if ((rc = set_smem<N, -1>()) || (rc = set_smem<N, 2>()) || (rc = set_smem<N, 3>()) || (rc = set_smem<N, 4>()) ||
+        (rc = set_smem<N, 5>()) || (rc = set_smem<N, 6>()))
+        return rc;
+    int occ = 0;
+    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_aos_kernel<N, -1>, CTA, smem_bytes<N>()));
+    int dev = 0, n_sm = 0;
+    DEDISP_CUDA_TRY(cudaGetDevice(&dev));
+    DEDISP_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    g_info[slot].ctas_per_sm = occ > 0 ? occ : 1;
+    g_info[slot].n_sm = n_sm;
+    g_info[slot].spec_bytes = sizeof(float2) * (size_t)g_info[slot].ctas_per_sm * n_sm * units_per_super_of<N>() * N;
+    return DEDISP_OK;
+}
+
+template <int N>
+int launch_one(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
+{
+    const int slot = slot_of(N);
+    long long grid = (long long)g_info[slot].ctas_per_sm * g_info[slot].n_sm;
+    if (grid > a.n_super) grid = a.n_super;
+    a.spec = p->d_spec;
+    const dim3 g((unsigned)grid), b(CTA);
+    switch (a.volt ? -1 : a.log2_nint) {  // n_int = 4 ... 64 (the five BASELINE configs) are specialised
+        case 2: fused_aos_kernel<N, 2><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        case 3: fused_aos_kernel<N, 3><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        case 4: fused_aos_kernel<N, 4><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        case 5: fused_aos_kernel<N, 5><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        case 6: fused_aos_kernel<N, 6><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        default: fused_aos_kernel<N, -1><<<g, b, smem_bytes<N>(), st>>>(a); break;
+    }
+    DEDISP_CUDA_TRY(cudaGetLastError());
+    return DEDISP_OK;
+}
+
+int dispatch(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
+{
+    switch (p->n_fft) {
+        case 1024: return launch_one<1024>(p, a, st);
+        case 2048: return launch_one<2048>(p, a, st);
+        case 4096: return launch_one<4096>(p, a, st);
+        case 8192: return launch_one<8192>(p, a, st);
+        case 16384: return launch_one<16384>(p, a, st);
+        default: return DEDISP_EINVAL;
+    }
+}
+
+int units_per_super(int n_fft)
+{
+    switch (n_fft) {
+        case 1024: return units_per_super_of<1024>(); case 2048: return units_per_super_of<2048>();
+        case 4096: return units_per_super_of<4096>(); case 8192: return units_per_super_of<8192>();
+        default: return units_per_super_of<16384>();
+    }
+}
+
+int base_args(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, AosArgs& a)
+{
+    const long long ups = units_per_super(p->n_fft), spc = (nb + ups - 1) / ups;
+    if (nb > 0x3fffffff || spc * p->n_chan > 0x7fffffff) return DEDISP_EINVAL;  // 32-bit item arithmetic in the kernel
+    a = AosArgs{};
+    a.xt = d_xt; a.xt_stride = xt_stride; a.chirp = p->d_chirp; a.tw = p->d_twiddle;
+    a.nb = (int)nb; a.spc = (int)spc; a.n_super = (int)(spc * p->n_chan); a.first_super = 0;
+    a.n_chan = p->n_chan; a.n_dm = p->n_dm; a.head = p->head; a.L = p->L;
+    int lg = 0;
+    while ((1 << lg) < p->n_int) ++lg;
+    a.log2_nint = lg;
+    return DEDISP_OK;
+}
+
+}  // namespace
+
+int dedisp_aos_supported(int n_fft) { return slot_of(n_fft) >= 0; }
+
+size_t dedisp_aos_spec_bytes(int n_fft)
+{
+    const int slot = slot_of(n_fft);
+    return slot < 0 ? 0 : g_info[slot].spec_bytes;
+}
+
+int dedisp_aos_init(void)
+{
+    if (g_init_done) return DEDISP_OK;
+    int rc;
+    if ((rc = init_one<1024>(0)) || (rc = init_one<2048>(1)) || (rc = init_one<4096>(2)) || (rc = init_one<8192>(3)) ||
+        (rc = init_one<16384>(4)))
+        return rc;
+    g_init_done = true;
+    return DEDISP_OK;
+}
+
+int dedisp_launch_aos(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
+                      long long out_stride, long long out_col0, cudaStream_t st)
+{
+    AosArgs a;
+    int rc = base_args(p, d_xt, xt_stride, nb, a);
+    if (rc != DEDISP_OK) return rc;
+    a.out = d_out; a.out_stride = out_stride; a.out_col0 = out_col0;
+    return dispatch(p, a, st);
+}
+
+int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
+                                    long long block, float* d_volt, cudaStream_t st)
+{
+    // the one super-item that holds (chan, block); blocks-per-channel = block + 1 is enough to address it
+    AosArgs a;
+    int rc = base_args(p, d_xt, xt_stride, block + 1, a);
+    if (rc != DEDISP_OK) return rc;
+    a.first_super = chan * a.spc + (int)(block / units_per_super(p->n_fft));
+    a.n_super = 1;
+    a.volt = reinterpret_cast<float2*>(d_volt);
+    a.volt_block = (int)block;
+    return dispatch(p, a, st);
+}
