@@ -39,7 +39,7 @@ N_SM, FP32_LANES_PER_SM = 148, 128   # B200: 148 SMs x 4 sub-partitions x 32 FP3
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full`
 # capture (profiles/), keyed by workload; None until a capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"gmrt32": 1.0417e9 + 0.4829e9}   # profiles/r1f_ncu_gmrt32.md
+NCU_TRAFFIC_BYTES = {"gmrt32": 1.0419e9 + 0.4826e9}   # profiles/r1h_ncu_gmrt32.md
 
 
 def parse_args():
@@ -387,7 +387,7 @@ def run_ours(args):
     abytes = n_units * algorithmic_bytes_per_unit(w.n_fft, L, plan.n_dm, w.n_int)
     achieved_tf = flops / (fused_ms * 1e-3) / 1e12
     roofline = {
-        "bound": "alu", "kernel": "fused_dedisp_kernel", "achieved": achieved_tf, "peak": fp32_peak_tf,
+        "bound": "alu", "kernel": "fused_aos_kernel", "achieved": achieved_tf, "peak": fp32_peak_tf,
         "unit": "TFLOP/s", "frac": achieved_tf / fp32_peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
         "peak_source": f"{N_SM} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 (FMA) x {sm_max:.0f} MHz "
                        f"(sm_max_mhz of MEASURED_PEAKS.json, {peaks_src})",

@@ -52,7 +52,7 @@ extern thread_local int g_dedisp_last_cuda;
 // (= 128 B) so every block start b*L (L % 32 == 0) stays 64 B aligned for vector / bulk loads.
 static inline long long dedisp_xt_stride(long long n_samp) { return (n_samp + 63) / 64 * 64; }
 
-// kernels.cu / fused.cu launchers (all enqueue only)
+// corner_turn.cu (all launchers enqueue only)
 // corner turn: int8 [n_samp][n_chan][2] -> int8 [n_chan][xt_stride][2], rows t0_dst.. of the destination
 int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int8_t* d_xt, long long xt_stride,
                               long long dst_t0, cudaStream_t st);
