@@ -321,3 +321,25 @@ def test_profile_hooks_time_both_kernels(dd, torch):
         plan.profile_enable(False)
         plan.execute(x)
         assert plan.profile_read()[2] == 0
+
+
+def test_repeated_calls_are_bitwise_identical(dd, torch):
+    """Every output is written by exactly one thread from values that only depend on its (dm, channel, block) unit, so
+    two calls on the same input must agree bit for bit; a missing barrier or a buffer reused too early would show up
+    here (compute-sanitizer is not available on this pool).  Large enough for every CTA to walk several super-items
+    with all four groups busy, and to change channel inside a CTA."""
+    w = datagen.WORKLOADS["gmrt32"]
+    n_chan = 512
+    with dd.dedisp_plan(n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int) as plan:
+        n_samp = 37 * plan.L + plan.head + plan.tail + 5          # 37 blocks: super-items of 4 leave one block over
+        x = torch.from_numpy(datagen.noise_only(n_samp, n_chan, seed=99)).cuda()
+        a = plan.execute(x).clone()
+        for _ in range(3):
+            b = plan.execute(x)
+            torch.cuda.synchronize()
+            assert torch.equal(a, b)
+        # the same blocks computed with a different block-to-group assignment (the input shifted by one block)
+        c = plan.execute(x[plan.L:].contiguous())
+        torch.cuda.synchronize()
+        per = plan.L // plan.n_int
+        assert torch.equal(a[:, :, per:], c)
