@@ -1,14 +1,23 @@
-// fused_aos.cu -- steps 1b-6 of the path for N_fft <= 4096, one (channel, block) unit per 256 threads (or fewer), every
-// complex number in one packed f32x2 register pair (fft_aos.cuh): unpack -> forward FFT -> chirp -> inverse FFT ->
-// |v|^2 -> integrate on FADD2/FMUL2/FFMA2 (Fig. 4).  HBM traffic: 2 B in,
-// 4/n_int B out per complex sample.
+// fused_aos.cu -- steps 1b-6 of the path in ONE kernel per call, for every built transform size: unpack -> forward
+// FFT -> chirp -> inverse FFT -> overlap discard -> |v|^2 -> integrate (Fig. 4).
+// A complex sample is read once from HBM as 2 bytes and leaves as 4/n_int bytes; everything in between stays in
+// registers and shared memory.  Every complex number is one packed f32x2 register pair (fft_aos.cuh), so the arithmetic
+// is FADD2/FMUL2/FFMA2.  The forward spectrum is computed once per (channel, block) and shared by all trial DMs.
 //
-// 16 elements per thread = 32 data registers, so ONE persistent 1024-thread CTA per SM holds FOUR groups of 256
-// threads, each with its own units, exchange buffers and named barrier: while one group is in a shared-memory
-// exchange the other three keep the FP32 pipe busy.  A CTA walks a contiguous range of "super-items" (4U consecutive
-// blocks of ONE channel, U = 1/2/4 units per group for N = 4096/2048/1024):
-//   * the channel's chirp row sits in shared memory and is reloaded only when the channel changes;
+// 16 elements per thread = 32 data registers (64 in all), N/16 threads per (channel, block) unit, ONE persistent
+// 1024-thread CTA per SM split into groups that own their units, exchange buffers and a named barrier: four groups of
+// 256 threads for N <= 4096 (1/2/4 units each), two of 512 for N = 8192, one of 1024 for N = 16384.  While one group is
+// in a shared-memory exchange the others keep the FP32 pipe busy.  A CTA walks a contiguous range of "super-items"
+// (consecutive blocks of ONE channel, one per unit slot):
+//   * for N <= 4096 the channel's chirp row sits in shared memory and is reloaded only when the channel changes
+//     (larger rows do not fit beside the exchange buffers and come from L2);
 //   * the int8 rows of the NEXT super-item are prefetched with cp.async while this one computes.
+// Barrier discipline (compute-sanitizer is not available on this pool, so it is spelled out): a group's staging rows
+// are written by cp.async issued after the first barrier of the forward transform (every thread of the group is then
+// past its unpack reads) and become visible at the barrier that ends the super-item (cp.async.wait_group 0 before it);
+// the exchange buffer is reused for the detected powers only after the last gather's barrier, and for the next
+// transform's scatter only after the epilogue's closing barrier; the chirp row is rewritten between two
+// __syncthreads() that all groups reach in the same loop iteration.
 #include "dedisp_internal.h"
 #include "fft_aos.cuh"
 
