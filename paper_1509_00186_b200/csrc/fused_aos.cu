@@ -104,8 +104,13 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
     const int lg_lpo = lgn - lg_chunk;
     const int n_work = a.L >> lg_chunk;
 
-    const int s_begin = a.first_super + (int)((long long)blockIdx.x * a.n_super / gridDim.x);
-    const int s_end = a.first_super + (int)((long long)(blockIdx.x + 1) * a.n_super / gridDim.x);
+    // Work split.  Chirp row in shared memory: a contiguous range per CTA, so the row is reloaded only at channel
+    // changes.  Chirp row from L2 (N > 4096): super-items dealt round-robin, so that at any moment all CTAs work on the
+    // same one or two channels and their chirp rows (8 B x N per trial DM) stay L2-resident instead of 148 different
+    // channels' worth of rows thrashing it.
+    const int s_step = CHIRP_SMEM ? 1 : (int)gridDim.x;
+    const int s_begin = a.first_super + (CHIRP_SMEM ? (int)((long long)blockIdx.x * a.n_super / gridDim.x) : (int)blockIdx.x);
+    const int s_end = a.first_super + (CHIRP_SMEM ? (int)((long long)(blockIdx.x + 1) * a.n_super / gridDim.x) : a.n_super);
 
     // stage the int8 rows of this thread's unit of super-item s: 2 x 16 B per thread (P:L270 framing: block b reads
     // rows b*L .. b*L+N-1; consecutive blocks overlap)
@@ -130,7 +135,7 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
         group_bar(bar_id, GROUP);
     }
 
-    for (int s = s_begin; s < s_end; ++s) {
+    for (int s = s_begin; s < s_end; s += s_step) {
         const int c = s / a.spc;
         const int b = (s - c * a.spc) * UPS + us;
         const bool live = b < a.nb;
@@ -152,7 +157,7 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
         // 2. forward FFT; once every thread of the group is past the unpack, the staging buffer is
         //    free for the next super-item's rows
         fft_aos<N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, -1>(x, t, sm, a.tw, bar_id, GROUP, [&] {
-            if (s + 1 < s_end) prefetch(s + 1);
+            if (s + s_step < s_end) prefetch(s + s_step);
         });
 
         float2* stash = a.spec + ((size_t)blockIdx.x * UPS + us) * N;
