@@ -72,6 +72,10 @@ def lib():
         L.oracle_dedisp_units.restype = C.c_longlong
         L.oracle_unpack_block.argtypes = [cp, C.c_void_p, C.c_int, C.c_longlong, C.c_int, C.c_void_p]
         L.oracle_unpack_block.restype = None
+        L.oracle_band_shifts.argtypes = [cp, C.c_int, C.c_void_p]
+        L.oracle_band_shifts.restype = None
+        L.oracle_band_sum.argtypes = [cp, C.c_void_p, C.c_longlong, C.c_longlong, C.c_void_p, C.c_longlong]
+        L.oracle_band_sum.restype = C.c_longlong
         _lib = L
     return _lib
 
@@ -220,3 +224,21 @@ def unpack_block(cfg: OracleConfig, x: np.ndarray, c: int, b: int) -> np.ndarray
     dst = np.empty((cfg.n_fft, 2), dtype=np.float64)
     lib().oracle_unpack_block(C.byref(cfg.c()), x.ctypes.data, c, b, l, dst.ctypes.data)
     return dst
+
+
+def band_shifts(cfg: OracleConfig, d: int) -> np.ndarray:
+    """Whole-output-sample delays of every channel relative to the earliest one (NEXT-3, reading R16)."""
+    sh = np.zeros(cfg.n_chan, dtype=np.int64)
+    lib().oracle_band_shifts(C.byref(cfg.c()), d, sh.ctypes.data)
+    return sh
+
+
+def band_sum(cfg: OracleConfig, out: np.ndarray) -> np.ndarray:
+    """out float64 [n_dm][n_chan][n_out] -> aligned band sum float64 [n_dm][n_series]."""
+    out = np.ascontiguousarray(out, dtype=np.float64)
+    assert out.ndim == 3 and out.shape[0] == cfg.n_dm and out.shape[1] == cfg.n_chan
+    n_out = out.shape[2]
+    series = np.zeros((cfg.n_dm, n_out), dtype=np.float64)
+    n_ser = lib().oracle_band_sum(C.byref(cfg.c()), out.ctypes.data, n_out, n_out, series.ctypes.data, n_out)
+    return np.ascontiguousarray(series[:, :n_ser])
+

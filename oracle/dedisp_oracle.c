@@ -453,3 +453,63 @@ void oracle_unpack_block(const oracle_cfg_t *cfg, const int8_t *in, int c, long 
         dst_re_im[2 * n + 1] = (double)p[1];
     }
 }
+
+/* ---------------------------------------------------------------------------
+ * NEXT-3: alignment of the coherently dedispersed
+ * sub-bands in time and band sum.
+ *
+ * "Appropriate time delays are then applied to align the pulses in the
+ * separate frequency channels, which are then added to produce a dedispersed
+ * time series."  P:L67: "coherently dedispersing each sub-band, followed by
+ * alignment of the individual sub-bands in time".
+ *
+ * Reading R16: after per-channel coherent dedispersion about the
+ * channel centre, channel c carries the pulse at the arrival time of its
+ * centre frequency f_c; relative to the highest channel it is late by
+ *     delay(d, c) = D * DM_d * (1/f_c^2 - 1/f_top^2)          (P:L39-41 delay law)
+ * seconds = delay * dv / n_int output samples.  Only whole output samples are
+ * shifted ("time delays", not phase ramps):
+ *     shift(d, c) = lround(delay * dv / n_int) - min_c' lround(...)   (>= 0, so a
+ *                   negative DM, whose lowest channel arrives first, works too)
+ *     series[d][j] = sum_c out[d][c][j + shift(d, c)],  j in [0, n_out - max_c shift)
+ * ------------------------------------------------------------------------- */
+void oracle_band_shifts(const oracle_cfg_t *cfg, int d, long long *shift /* [n_chan] */)
+{
+    double f_top = oracle_chan_freq(cfg, cfg->n_chan - 1);
+    double dv = oracle_chan_width(cfg);
+    long long lo = 0;
+    for (int c = 0; c < cfg->n_chan; ++c) {
+        double f_c = oracle_chan_freq(cfg, c);
+        double delay_s = ORACLE_D_HZ2_S * cfg->dm[d] * (1.0 / (f_c * f_c) - 1.0 / (f_top * f_top));
+        shift[c] = llround(delay_s * dv / (double)cfg->n_int);
+        if (c == 0 || shift[c] < lo) lo = shift[c];
+    }
+    for (int c = 0; c < cfg->n_chan; ++c) shift[c] -= lo;
+}
+
+/* out [n_dm][n_chan][out_stride] (first n_out columns valid) -> series [n_dm][series_stride].
+ * Returns n_series = n_out - (largest shift over all DMs and channels), the same length for every DM so that
+ * the rows share a time axis; 0 if that is not positive. */
+long long oracle_band_sum(const oracle_cfg_t *cfg, const double *out, long long out_stride, long long n_out,
+                          double *series, long long series_stride)
+{
+    int C = cfg->n_chan;
+    long long *shift = (long long *)malloc(sizeof(long long) * (size_t)C * cfg->n_dm);
+    long long max_shift = 0;
+    for (int d = 0; d < cfg->n_dm; ++d) {
+        oracle_band_shifts(cfg, d, shift + (size_t)d * C);
+        for (int c = 0; c < C; ++c)
+            if (shift[(size_t)d * C + c] > max_shift) max_shift = shift[(size_t)d * C + c];
+    }
+    long long n_ser = n_out - max_shift;
+    if (n_ser <= 0 || series_stride < n_ser) { free(shift); return 0; }
+    for (int d = 0; d < cfg->n_dm; ++d)
+        for (long long j = 0; j < n_ser; ++j) {
+            double acc = 0.0;
+            for (int c = 0; c < C; ++c)
+                acc += out[((size_t)d * C + c) * out_stride + j + shift[(size_t)d * C + c]];
+            series[(size_t)d * series_stride + j] = acc;
+        }
+    free(shift);
+    return n_ser;
+}

@@ -479,3 +479,81 @@ def test_p14_injected_pulsar_is_sharpest_at_its_dm():
                 assert prof.argmax() == 0
         peaks[dm] = np.mean(tops)
     assert peaks[10.0] > 1.3 * peaks[5.0] > 1.3 * 1.2 * peaks[0.0]
+
+
+# ----------------------------------------------------------------------------- P15-P17: band alignment + sum (NEXT-3)
+def test_p15_band_shifts_follow_the_printed_delay_law():
+    """P:L39-41 / P:L117: the delay between two frequencies is D * DM * (f1^-2 - f2^-2) with D printed in MHz/us
+    units (golden file); the oracle's shifts (computed in Hz/s) must be that delay in whole output samples."""
+    for name in ("tiny", "gmrt32", "lowfreq"):
+        w = datagen.WORKLOADS[name]
+        cfg = oracle.OracleConfig(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
+        sh = oracle.band_shifts(cfg, 0)
+        f_mhz = datagen.chan_freqs_hz(w) / 1e6
+        delay_us = GOLD["D_MHZ2_US"] * w.dm_trials[0] * (f_mhz ** -2 - f_mhz[-1] ** -2)        # paper's units
+        expect = delay_us * 1e-6 * w.chan_width_hz / w.n_int                                 # output samples
+        assert sh[-1] == 0 and sh.min() == 0
+        assert np.all(np.diff(sh) <= 0)                        # lower channels arrive later
+        assert np.abs(sh - expect).max() <= 0.5 + 1e-6         # nearest whole sample
+        # adjacent channels differ by the dispersion smear between their centres (an independent oracle helper)
+        fc = datagen.chan_freqs_hz(w)
+        smear = np.array([oracle.smear_seconds(w.dm_trials[0], fc[c], fc[c + 1]) for c in range(w.n_chan - 1)])
+        assert np.abs(-np.diff(sh) - smear * w.chan_width_hz / w.n_int).max() <= 1.0 + 1e-6
+
+
+def test_p15_negative_dm_mirrors_the_shifts():
+    cfg_p = cfg_tiny(dm=(10.0,))
+    cfg_n = cfg_tiny(dm=(-10.0,))
+    sp, sn = oracle.band_shifts(cfg_p, 0), oracle.band_shifts(cfg_n, 0)
+    assert sn.min() == 0 and sn[0] == 0 and np.all(np.diff(sn) >= 0)
+    assert np.abs((sp.max() - sp) - sn).max() <= 1
+
+
+def test_p16_band_sum_integer_closed_form():
+    """A unit impulse placed in every channel at its own arrival sample sums to exactly C at one sample and to 0
+    elsewhere; DM = 0 reduces the band sum to the plain sum over channels."""
+    cfg = cfg_tiny(dm=(10.0, 0.0, -7.0))
+    n_out, j0 = 900, 123
+    out = np.zeros((3, cfg.n_chan, n_out))
+    for d in range(3):
+        sh = oracle.band_shifts(cfg, d)
+        out[d, np.arange(cfg.n_chan), j0 + sh] = 1.0
+    s = oracle.band_sum(cfg, out)
+    max_shift = max(int(oracle.band_shifts(cfg, d).max()) for d in range(3))
+    assert s.shape == (3, n_out - max_shift)
+    for d in range(3):
+        assert s[d, j0] == cfg.n_chan and s[d].sum() == cfg.n_chan
+    rng = np.random.default_rng(3)
+    r = rng.normal(size=(3, cfg.n_chan, n_out))
+    s = oracle.band_sum(cfg, r)
+    assert np.allclose(s[1], r[1].sum(0)[: s.shape[1]], rtol=0, atol=1e-12)
+    # brute force for the dispersed rows, written out index by index
+    sh0 = oracle.band_shifts(cfg, 0)
+    for j in (0, 17, s.shape[1] - 1):
+        assert abs(s[0, j] - sum(r[0, c, j + sh0[c]] for c in range(cfg.n_chan))) < 1e-12
+
+
+def test_p17_band_sum_raises_the_pulse_above_a_single_channel():
+    """Science sanity for the whole chain (statistical): coherent dedispersion per channel + alignment + band sum of
+    the tiny workload gives a folded pulse whose signal-to-noise beats a single channel's by roughly sqrt(C), and
+    summing WITHOUT the alignment (DM 0 shifts) smears it away."""
+    w = datagen.WORKLOADS["tiny"]
+    x = datagen.generate(w)
+    cfg = oracle.OracleConfig(w.n_chan, w.bw_hz, w.f_center_hz, (w.pulse_dm,), w.n_fft, w.n_int)
+    head, tail, L = oracle.framing(cfg)
+    out = oracle.dedisp(cfg, x, n_threads=os.cpu_count() or 1)
+
+    def snr(series):
+        t = (head + np.arange(series.size) * w.n_int + 0.5 * w.n_int) / w.chan_width_hz
+        nbin = 39
+        b = np.minimum((np.mod(t, w.pulse_period_s) / w.pulse_period_s * nbin).astype(int), nbin - 1)
+        prof = np.bincount(b, series, nbin) / np.maximum(np.bincount(b, None, nbin), 1)
+        off = np.sort(prof)[: nbin // 2]
+        return (prof.max() - np.median(prof)) / off.std()
+
+    aligned = oracle.band_sum(cfg, out)[0]
+    cfg0 = oracle.OracleConfig(w.n_chan, w.bw_hz, w.f_center_hz, (0.0,), w.n_fft, w.n_int)
+    unaligned = oracle.band_sum(cfg0, out)[0]
+    single = out[0, w.n_chan - 1]
+    assert snr(aligned) > 4.0 * snr(single)           # sqrt(64) = 8 in the ideal case
+    assert snr(aligned) > 3.0 * snr(unaligned)
