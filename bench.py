@@ -377,6 +377,28 @@ def run_ours(args):
         except Exception as exc:            # the reference point must never take the bench down
             cufft_ref = {"error": repr(exc)[:200]}
 
+    # ---- sub-band alignment + band sum on the step's output (HBM-bound; not part of the step) ------
+    band = None
+    if rank == 0:
+        n_ser = plan.band_samples(n_out)
+        if n_ser > 0:
+            d_series = torch.empty((plan.n_dm, n_ser), dtype=torch.float32, device="cuda")
+            for _ in range(3):
+                plan.band_sum(d_out, d_series)
+            torch.cuda.synchronize()
+            b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            b0.record()
+            for _ in range(args.steps):
+                plan.band_sum(d_out, d_series)
+            b1.record()
+            torch.cuda.synchronize()
+            b_ms = b0.elapsed_time(b1) / args.steps
+            b_bytes = 4.0 * plan.n_dm * n_ser * (w.n_chan + 1)
+            band = {"kernel": "band_sum_kernel", "ms_per_launch": b_ms, "n_series": n_ser,
+                    "algorithmic_bytes_per_launch": b_bytes, "achieved_gbs": b_bytes / (b_ms * 1e-3) / 1e9,
+                    "note": "output of the step is 510 MB: partly L2-resident between launches" if d_out.numel() * 4 < 1e9 else ""}
+            del d_series
+
     # ---- roofline of the dominant (fused) kernel --------------------------------------------------------------------
     peaks, peaks_src = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
@@ -436,7 +458,7 @@ def run_ours(args):
                          "input smaller than 2x L2: numbers include L2 hits",
                    "sharding": "one workload-sized batch per rank, no data-path collective"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps,
-        "roofline": roofline, "cpu_baseline": cpu, "cufft_reference_point": cufft_ref,
+        "roofline": roofline, "cpu_baseline": cpu, "cufft_reference_point": cufft_ref, "next_rows": {"band_sum": band},
         "checksum_mean_first_1000": checksum,
     }
     print(json.dumps(line), flush=True)

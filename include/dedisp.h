@@ -125,6 +125,24 @@ int dedisp_stream_end(dedisp_plan_t plan);
 int dedisp_profile_enable(dedisp_plan_t plan, int on);
 int dedisp_profile_read(dedisp_plan_t plan, double* ms_corner_turn, double* ms_fused, int* n_calls);
 
+/*
+ * Alignment of the coherently dedispersed sub-bands in time and band sum ("Appropriate time delays are then
+ * applied to align the pulses in the separate frequency channels, which are then added to produce a dedispersed time
+ * series"; "coherently dedispersing each sub-band, followed by alignment of the individual sub-bands in time").
+ * Reading R16: channel c is late against the highest channel by D*DM_d*(1/f_c^2 - 1/f_top^2) seconds; in
+ * whole output samples  shift(d,c) = lround(delay*dv/n_int) - min over c  (>= 0; negative DMs work too), and
+ *     series[d][j] = sum_c out[d][c][j + shift(d,c)],   j in [0, n_out - max shift over all d, c).
+ *   dedisp_band_samples  series length for n_out output samples per (dm, channel); 0 if n_out <= the largest shift.
+ *   dedisp_band_shifts   HOST int64 [n_chan]: shift(d, .).
+ *   dedisp_band_sum      d_out DEVICE float [n_dm][n_chan][out_stride] (as written by dedisp_execute), first n_out
+ *                        columns valid; d_series DEVICE float [n_dm][series_stride], series_stride >= the series
+ *                        length.  Enqueues one kernel on cuda_stream.  Errors: EINVAL, ESHORT (n_out too short), ECUDA.
+ */
+long long dedisp_band_samples(dedisp_plan_t plan, long long n_out);
+int dedisp_band_shifts(dedisp_plan_t plan, int d, long long* h_shift);
+int dedisp_band_sum(dedisp_plan_t plan, const float* d_out, long long out_stride, long long n_out, float* d_series,
+                    long long series_stride, void* cuda_stream);
+
 int dedisp_destroy(dedisp_plan_t plan);
 
 const char* dedisp_strerror(int code);

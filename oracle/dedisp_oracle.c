@@ -44,6 +44,7 @@
  *   R10 int8 two's complement, re then im, layout [t][chan][2].
  *   R11 detection |v|^2 = re^2 + im^2; integration = plain sum of n_int samples.
  *   R12 no zero padding; output j covers input times head + j*n_int ...
+ *   R16 sub-band alignment in whole output samples against the top channel (oracle_band_sum).
  */
 #include <complex.h>
 #include <math.h>

@@ -16,7 +16,7 @@ TAPER = {"none": 0, "hann": 1, "welch": 2}
 SYMBOLS = (
     "dedisp_framing", "dedisp_plan", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
     "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_profile_enable",
-    "dedisp_profile_read", "dedisp_destroy",
+    "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_destroy",
     "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
 )
 
@@ -55,6 +55,10 @@ def _load() -> C.CDLL:
     L.dedisp_stream_end.argtypes = [vp]
     L.dedisp_profile_enable.argtypes = [vp, C.c_int]
     L.dedisp_profile_read.argtypes = [vp, dp, dp, ip]
+    L.dedisp_band_samples.argtypes = [vp, ll]
+    L.dedisp_band_samples.restype = ll
+    L.dedisp_band_shifts.argtypes = [vp, C.c_int, C.POINTER(ll)]
+    L.dedisp_band_sum.argtypes = [vp, vp, ll, ll, vp, ll, vp]
     L.dedisp_destroy.argtypes = [vp]
     L.dedisp_strerror.argtypes = [C.c_int]
     L.dedisp_strerror.restype = C.c_char_p
@@ -166,6 +170,32 @@ class Plan:
 
     def stream_end(self) -> None:
         _check(_lib.dedisp_stream_end(self._h), "dedisp_stream_end")
+
+    # -- sub-band alignment + band sum ------------------------------------------------------------------------
+    def band_samples(self, n_out: int) -> int:
+        return int(_lib.dedisp_band_samples(self._h, n_out))
+
+    def band_shifts(self, d: int):
+        import numpy as np
+        sh = (C.c_longlong * self.n_chan)()
+        _check(_lib.dedisp_band_shifts(self._h, d, sh), "dedisp_band_shifts")
+        return np.asarray(list(sh), dtype=np.int64)
+
+    def band_sum(self, d_out, d_series=None, stream=None):
+        """d_out: CUDA float32 [n_dm][n_chan][n_out] (from execute) -> CUDA float32 [n_dm][n_series]."""
+        import torch
+        assert d_out.is_cuda and d_out.dtype == torch.float32 and d_out.is_contiguous()
+        assert d_out.dim() == 3 and d_out.shape[0] == self.n_dm and d_out.shape[1] == self.n_chan
+        n_out = d_out.shape[2]
+        n_ser = self.band_samples(n_out)
+        if d_series is None:
+            d_series = torch.empty((self.n_dm, max(n_ser, 0)), dtype=torch.float32, device=d_out.device)
+        assert d_series.is_cuda and d_series.dtype == torch.float32 and d_series.is_contiguous()
+        assert d_series.dim() == 2 and d_series.shape[0] == self.n_dm
+        st = torch.cuda.current_stream(d_out.device).cuda_stream if stream is None else stream
+        _check(_lib.dedisp_band_sum(self._h, d_out.data_ptr(), n_out, n_out, d_series.data_ptr(), d_series.shape[1], st),
+               "dedisp_band_sum")
+        return d_series
 
     # -- kernel timing ----------------------------------------------------------------------------------------
     def profile_enable(self, on: bool = True) -> None:

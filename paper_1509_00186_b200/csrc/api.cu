@@ -30,6 +30,8 @@ static void free_plan(dedisp_plan_s* p)
     if (p->d_twiddle) cudaFree(p->d_twiddle);
     if (p->d_xt) cudaFree(p->d_xt);
     if (p->d_spec) cudaFree(p->d_spec);
+    if (p->d_band_shift) cudaFree(p->d_band_shift);
+    free(p->band_shift);
     if (p->prof_ev) {
         for (int i = 0; i < DEDISP_PROF_MAX * 3; ++i) cudaEventDestroy(p->prof_ev[i]);
         free(p->prof_ev);
@@ -78,6 +80,26 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     if (!p->dm) { free_plan(p); return DEDISP_ENOMEM; }
     memcpy(p->dm, dm, sizeof(double) * n_dm);
 
+    {   // band alignment (R16): delay of channel c against the top channel in whole output samples, minimum removed
+        p->band_shift = (long long*)malloc(sizeof(long long) * (size_t)n_dm * n_chan);
+        if (!p->band_shift) { free_plan(p); return DEDISP_ENOMEM; }
+        const double dv = bw_hz / n_chan, f_top = f_center_hz + 0.5 * bw_hz - 0.5 * dv;
+        p->band_max_shift = 0;
+        for (int d = 0; d < n_dm; ++d) {
+            long long* sh = p->band_shift + (size_t)d * n_chan;
+            long long lo = 0;
+            for (int c = 0; c < n_chan; ++c) {
+                const double fc = f_center_hz - 0.5 * bw_hz + ((double)c + 0.5) * dv;
+                const double delay_s = DEDISP_D_HZ2_S * dm[d] * (1.0 / (fc * fc) - 1.0 / (f_top * f_top));
+                sh[c] = llround(delay_s * dv / (double)n_int);
+                if (c == 0 || sh[c] < lo) lo = sh[c];
+            }
+            for (int c = 0; c < n_chan; ++c) {
+                sh[c] -= lo;
+                if (sh[c] > p->band_max_shift) p->band_max_shift = sh[c];
+            }
+        }
+    }
     double* d_dm = nullptr;
     auto fail = [&](int code) { if (d_dm) cudaFree(d_dm); free_plan(p); return code; };
 #define PLAN_TRY(expr)                                                                           \
@@ -94,6 +116,16 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     PLAN_TRY(cudaMalloc(&p->d_twiddle, sizeof(float2) * (size_t)n_fft));
     if (n_dm > 1)
         PLAN_TRY(cudaMalloc(&p->d_spec, dedisp_aos_spec_bytes(n_fft)));
+    if (p->band_max_shift < 0x7fffffffll) {  // device copy as int32 (a shift that large leaves no series anyway)
+        int* tmp = (int*)malloc(sizeof(int) * (size_t)n_dm * n_chan);
+        if (!tmp) return fail(DEDISP_ENOMEM);
+        for (size_t i = 0; i < (size_t)n_dm * n_chan; ++i) tmp[i] = (int)p->band_shift[i];
+        cudaError_t e1 = cudaMalloc(&p->d_band_shift, sizeof(int) * (size_t)n_dm * n_chan);
+        if (e1 == cudaSuccess)
+            e1 = cudaMemcpy(p->d_band_shift, tmp, sizeof(int) * (size_t)n_dm * n_chan, cudaMemcpyHostToDevice);
+        free(tmp);
+        PLAN_TRY(e1);
+    }
     PLAN_TRY(cudaMalloc(&d_dm, sizeof(double) * n_dm));
     PLAN_TRY(cudaMemcpy(d_dm, p->dm, sizeof(double) * n_dm, cudaMemcpyHostToDevice));
     rc = dedisp_launch_chirp_table(p, d_dm, 0);
@@ -210,6 +242,32 @@ extern "C" int dedisp_execute(dedisp_plan_t p, const int8_t* d_in, long long n_s
     // only the rows that complete blocks are needed: nb*L + head + tail
     const long long used = nb * p->L + p->head + p->tail;
     return dedisp_enqueue_chunk(p, d_in, used, p->d_xt, stride, 0, nb, d_out, out_stride, st, nullptr);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// sub-band alignment + band sum
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" long long dedisp_band_samples(dedisp_plan_t p, long long n_out)
+{
+    if (!p) return DEDISP_EINVAL;
+    return n_out > p->band_max_shift ? n_out - p->band_max_shift : 0;
+}
+
+extern "C" int dedisp_band_shifts(dedisp_plan_t p, int d, long long* h_shift)
+{
+    if (!p || !h_shift || d < 0 || d >= p->n_dm) return DEDISP_EINVAL;
+    memcpy(h_shift, p->band_shift + (size_t)d * p->n_chan, sizeof(long long) * p->n_chan);
+    return DEDISP_OK;
+}
+
+extern "C" int dedisp_band_sum(dedisp_plan_t p, const float* d_out, long long out_stride, long long n_out,
+                               float* d_series, long long series_stride, void* cuda_stream)
+{
+    if (!p || !d_out || !d_series || n_out <= 0 || out_stride < n_out || !p->d_band_shift) return DEDISP_EINVAL;
+    const long long n_ser = dedisp_band_samples(p, n_out);
+    if (n_ser <= 0) return DEDISP_ESHORT;
+    if (series_stride < n_ser) return DEDISP_EINVAL;
+    return dedisp_launch_band_sum(p, d_out, out_stride, d_series, series_stride, n_ser, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int dedisp_destroy(dedisp_plan_t p)

@@ -29,6 +29,10 @@ struct dedisp_plan_s {
     float2* d_spec;     // [resident CTAs][units per CTA][n_fft] forward-spectrum stash shared by the trial DMs (n_dm > 1)
     int8_t* d_xt;
     long long xt_cap_samp;  // samples per row the scratch can hold
+    // band alignment (R16): whole-output-sample delay of every channel, host and device copies [n_dm][n_chan]
+    long long* band_shift;
+    int* d_band_shift;
+    long long band_max_shift;
     dedisp_stream_state* stream;
     // kernel timing (dedisp_profile_enable): 3 events per call -- before corner turn, between, after fused
     int prof_on, prof_n;
@@ -79,5 +83,8 @@ int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows,
                          long long dst_t0, long long nb, float* d_out, long long out_stride, cudaStream_t st,
                          cudaEvent_t after_corner_turn);
 long long dedisp_n_blocks(const dedisp_plan_s* p, long long n_samp);
+// band_sum.cu
+int dedisp_launch_band_sum(const dedisp_plan_s* p, const float* d_out, long long out_stride, float* d_series,
+                           long long series_stride, long long n_series, cudaStream_t st);
 // stream.cu
 void dedisp_stream_free(dedisp_plan_s* p);
