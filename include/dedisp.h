@@ -98,6 +98,15 @@ int dedisp_execute(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, flo
                    void* cuda_stream);
 
 /*
+ * Second polarisation.  P:L258: the two polarisations of the beam are dedispersed separately "to
+ * allow one to combine the signals from the two polarisations after detection".  Same as dedisp_execute, but the
+ * integrated intensities are ADDED to what d_out already holds (stream order: after an earlier dedisp_execute on the
+ * same stream for the first polarisation), so that d_out ends up as the total intensity |v_1|^2 + |v_2|^2.
+ */
+int dedisp_execute_add(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, float* d_out, long long out_stride,
+                       void* cuda_stream);
+
+/*
  * Streaming form (host->device copy, compute and device->host copy overlapped on three streams; P:L270:
  * the samples lost at a block edge are prefixed to the next block).  Push consecutive chunks of the same observation;
  * the plan keeps the unconsumed tail on the device so that the concatenated output equals a one-shot call on the

@@ -15,6 +15,7 @@ TAPER = {"none": 0, "hann": 1, "welch": 2}
 # every symbol include/dedisp.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "dedisp_framing", "dedisp_plan", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
+    "dedisp_execute_add",
     "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_profile_enable",
     "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_destroy",
     "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
@@ -49,6 +50,7 @@ def _load() -> C.CDLL:
     L.dedisp_out_samples.restype = ll
     L.dedisp_reserve.argtypes = [vp, ll]
     L.dedisp_execute.argtypes = [vp, vp, ll, vp, ll, vp]
+    L.dedisp_execute_add.argtypes = [vp, vp, ll, vp, ll, vp]
     L.dedisp_stream_begin.argtypes = [vp, ll]
     L.dedisp_stream_push.argtypes = [vp, vp, ll, vp, ll, C.POINTER(ll)]
     L.dedisp_stream_sync.argtypes = [vp]
@@ -125,11 +127,13 @@ class Plan:
         _check(_lib.dedisp_reserve(self._h, n_samp), "dedisp_reserve")
 
     # -- one-shot ---------------------------------------------------------------------------------------------
-    def execute(self, d_in, d_out=None, stream=None):
-        """d_in: CUDA int8 tensor [n_samp][n_chan][2]; returns/fills CUDA float32 [n_dm][n_chan][n_out]."""
+    def execute(self, d_in, d_out=None, stream=None, add: bool = False):
+        """d_in: CUDA int8 tensor [n_samp][n_chan][2]; returns/fills CUDA float32 [n_dm][n_chan][n_out].
+        add=True: dedisp_execute_add, the intensities are added to d_out (second polarisation)."""
         import torch
         assert d_in.is_cuda and d_in.dtype == torch.int8 and d_in.is_contiguous()
         assert d_in.dim() == 3 and d_in.shape[1] == self.n_chan and d_in.shape[2] == 2
+        assert not add or d_out is not None, "add=True needs the first polarisation's output"
         n_samp = d_in.shape[0]
         n_out = self.out_samples(n_samp)
         if d_out is None:
@@ -137,8 +141,8 @@ class Plan:
         assert d_out.is_cuda and d_out.dtype == torch.float32 and d_out.is_contiguous()
         assert d_out.dim() == 3 and d_out.shape[0] == self.n_dm and d_out.shape[1] == self.n_chan
         st = torch.cuda.current_stream(d_in.device).cuda_stream if stream is None else stream
-        _check(_lib.dedisp_execute(self._h, d_in.data_ptr(), n_samp, d_out.data_ptr(), d_out.shape[2], st),
-               "dedisp_execute")
+        fn = _lib.dedisp_execute_add if add else _lib.dedisp_execute
+        _check(fn(self._h, d_in.data_ptr(), n_samp, d_out.data_ptr(), d_out.shape[2], st), "dedisp_execute")
         return d_out
 
     def execute_ptr(self, in_ptr: int, n_samp: int, out_ptr: int, out_stride: int, stream: int = 0) -> None:

@@ -162,7 +162,7 @@ static long long n_blocks(const dedisp_plan_s* p, long long n_samp) { return ded
 // (the streaming path frees its staging buffer there).
 int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows, int8_t* d_xt, long long xt_stride,
                          long long dst_t0, long long nb, float* d_out, long long out_stride, cudaStream_t st,
-                         cudaEvent_t after_corner_turn)
+                         cudaEvent_t after_corner_turn, int accumulate)
 {
     cudaEvent_t* ev = nullptr;
     if (p->prof_on && p->prof_n < DEDISP_PROF_MAX) ev = p->prof_ev + 3 * (p->prof_n++);
@@ -172,7 +172,7 @@ int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows,
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[1], st));
     if (after_corner_turn) DEDISP_CUDA_TRY(cudaEventRecord(after_corner_turn, st));
     if (nb > 0) {
-        rc = dedisp_launch_aos(p, d_xt, xt_stride, nb, d_out, out_stride, 0, st);
+        rc = dedisp_launch_aos(p, d_xt, xt_stride, nb, d_out, out_stride, 0, accumulate, st);
         if (rc != DEDISP_OK) return rc;
     }
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[2], st));
@@ -227,8 +227,8 @@ extern "C" int dedisp_reserve(dedisp_plan_t p, long long n_samp)
     return DEDISP_OK;
 }
 
-extern "C" int dedisp_execute(dedisp_plan_t p, const int8_t* d_in, long long n_samp, float* d_out,
-                              long long out_stride, void* cuda_stream)
+static int execute_impl(dedisp_plan_t p, const int8_t* d_in, long long n_samp, float* d_out, long long out_stride,
+                        void* cuda_stream, int accumulate)
 {
     if (!p || !d_in || n_samp <= 0) return DEDISP_EINVAL;
     const long long nb = n_blocks(p, n_samp);
@@ -241,7 +241,19 @@ extern "C" int dedisp_execute(dedisp_plan_t p, const int8_t* d_in, long long n_s
     const long long stride = p->xt_cap_samp;
     // only the rows that complete blocks are needed: nb*L + head + tail
     const long long used = nb * p->L + p->head + p->tail;
-    return dedisp_enqueue_chunk(p, d_in, used, p->d_xt, stride, 0, nb, d_out, out_stride, st, nullptr);
+    return dedisp_enqueue_chunk(p, d_in, used, p->d_xt, stride, 0, nb, d_out, out_stride, st, nullptr, accumulate);
+}
+
+extern "C" int dedisp_execute(dedisp_plan_t p, const int8_t* d_in, long long n_samp, float* d_out,
+                              long long out_stride, void* cuda_stream)
+{
+    return execute_impl(p, d_in, n_samp, d_out, out_stride, cuda_stream, 0);
+}
+
+extern "C" int dedisp_execute_add(dedisp_plan_t p, const int8_t* d_in, long long n_samp, float* d_out,
+                                  long long out_stride, void* cuda_stream)
+{
+    return execute_impl(p, d_in, n_samp, d_out, out_stride, cuda_stream, 1);
 }
 
 // ---------------------------------------------------------------------------------------------------------------

@@ -62,8 +62,9 @@ int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, 
                               long long dst_t0, cudaStream_t st);
 // fused_aos.cu: fused unpack -> forward FFT -> chirp -> inverse FFT -> discard -> detect -> integrate over nb blocks of
 // every channel (all enqueue only):  out[d][c][out_col0 + b*L/n_int + j]
+// accumulate != 0: add to d_out instead of overwriting it
 int dedisp_launch_aos(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
-                      long long out_stride, long long out_col0, cudaStream_t st);
+                      long long out_stride, long long out_col0, int accumulate, cudaStream_t st);
 int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
                                     long long block, float* d_volt, cudaStream_t st);
 int dedisp_aos_supported(int n_fft);
@@ -81,7 +82,7 @@ int dedisp_framing_impl(int n_chan, double bw, double F, const double* dm, int n
 // api.cu: corner turn + fused kernel on `st` with the optional profiling events around them
 int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows, int8_t* d_xt, long long xt_stride,
                          long long dst_t0, long long nb, float* d_out, long long out_stride, cudaStream_t st,
-                         cudaEvent_t after_corner_turn);
+                         cudaEvent_t after_corner_turn, int accumulate = 0);
 long long dedisp_n_blocks(const dedisp_plan_s* p, long long n_samp);
 // band_sum.cu
 int dedisp_launch_band_sum(const dedisp_plan_s* p, const float* d_out, long long out_stride, float* d_series,

@@ -44,6 +44,7 @@ struct AosArgs {
     const float2* tw;      // [N] exp(-2 pi i m / N)
     float* out;            // [n_dm][n_chan][out_stride]
     long long out_stride, out_col0;
+    int accumulate;        // add to out instead of overwriting it (second polarisation)
     float2* spec;          // [gridDim.x][4U][N] forward-spectrum stash, used when n_dm > 1
     float2* volt;          // debug: [n_dm][L] voltages of block volt_block, else nullptr
     int volt_block;
@@ -219,7 +220,8 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
                     }
                 }
                 for (int off = 1; off < (1 << lg_lpo); off <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-                if (live && id < n_work && (id & ((1 << lg_lpo) - 1)) == 0) dst[id >> lg_lpo] = acc;
+                if (live && id < n_work && (id & ((1 << lg_lpo) - 1)) == 0)
+                    dst[id >> lg_lpo] = a.accumulate ? dst[id >> lg_lpo] + acc : acc;
             }
             // one barrier for two hand-overs: the powers live in the exchange buffer of the next transform, and the
             // rows prefetched for the next super-item (issued during this one's first exchange) become visible
@@ -342,12 +344,12 @@ int dedisp_aos_init(void)
 }
 
 int dedisp_launch_aos(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
-                      long long out_stride, long long out_col0, cudaStream_t st)
+                      long long out_stride, long long out_col0, int accumulate, cudaStream_t st)
 {
     AosArgs a;
     int rc = base_args(p, d_xt, xt_stride, nb, a);
     if (rc != DEDISP_OK) return rc;
-    a.out = d_out; a.out_stride = out_stride; a.out_col0 = out_col0;
+    a.out = d_out; a.out_stride = out_stride; a.out_col0 = out_col0; a.accumulate = accumulate;
     return dispatch(p, a, st);
 }
 

@@ -343,3 +343,21 @@ def test_repeated_calls_are_bitwise_identical(dd, torch):
         torch.cuda.synchronize()
         per = plan.L // plan.n_int
         assert torch.equal(a[:, :, per:], c)
+
+
+@pytest.mark.parametrize("n_fft,n_int,dm,n_chan", [(4096, 4, (71.0,), 6), (1024, 16, (10.0, 5.0), 9), (16384, 32, (150.0,), 2)])
+def test_two_polarisations_add_after_detection(dd, torch, n_fft, n_int, dm, n_chan):
+    """SURVEY 8(f) NEXT-4, P:L258 ("combine the signals from the two polarisations after detection"):
+    dedisp_execute on polarisation 1, dedisp_execute_add on polarisation 2 == oracle(pol 1) + oracle(pol 2)."""
+    bw = 62.5e3 * n_chan
+    cfg = oracle.OracleConfig(n_chan, bw, 325e6 if n_fft < 16384 else 150e6, dm, n_fft, n_int)
+    head, tail, L = oracle.framing(cfg)
+    n_samp = 3 * L + head + tail + 17
+    x1 = datagen.noise_only(n_samp, n_chan, seed=1000 + n_fft)
+    x2 = datagen.noise_only(n_samp, n_chan, seed=2000 + n_fft)
+    ref = oracle.dedisp(cfg, x1, n_threads=NT) + oracle.dedisp(cfg, x2, n_threads=NT)
+    with dd.dedisp_plan(n_chan, bw, cfg.f_center_hz, dm, n_fft, n_int) as plan:
+        out = plan.execute(torch.from_numpy(x1).cuda())
+        plan.execute(torch.from_numpy(x2).cuda(), out, add=True)
+        torch.cuda.synchronize()
+        assert_parity(out.cpu().numpy(), ref, L // n_int)
