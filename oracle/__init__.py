@@ -76,6 +76,9 @@ def lib():
         L.oracle_band_shifts.restype = None
         L.oracle_band_sum.argtypes = [cp, C.c_void_p, C.c_longlong, C.c_longlong, C.c_void_p, C.c_longlong]
         L.oracle_band_sum.restype = C.c_longlong
+        L.oracle_fold.argtypes = [C.c_void_p, C.c_longlong, C.c_double, C.c_double, C.c_double, C.c_int, C.c_void_p,
+                                  C.c_void_p]
+        L.oracle_fold.restype = None
         _lib = L
     return _lib
 
@@ -241,4 +244,13 @@ def band_sum(cfg: OracleConfig, out: np.ndarray) -> np.ndarray:
     series = np.zeros((cfg.n_dm, n_out), dtype=np.float64)
     n_ser = lib().oracle_band_sum(C.byref(cfg.c()), out.ctypes.data, n_out, n_out, series.ctypes.data, n_out)
     return np.ascontiguousarray(series[:, :n_ser])
+
+
+def fold(series, t0_s: float, dt_s: float, period_s: float, n_bins: int):
+    """Fold a time series at `period_s` (reading R17): (sum per phase bin, samples per phase bin)."""
+    series = np.ascontiguousarray(series, dtype=np.float64).reshape(-1)
+    s = np.zeros(n_bins, dtype=np.float64)
+    n = np.zeros(n_bins, dtype=np.int64)
+    lib().oracle_fold(series.ctypes.data, series.size, t0_s, dt_s, period_s, n_bins, s.ctypes.data, n.ctypes.data)
+    return s, n
 

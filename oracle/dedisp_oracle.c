@@ -514,3 +514,27 @@ long long oracle_band_sum(const oracle_cfg_t *cfg, const double *out, long long 
     free(shift);
     return n_ser;
 }
+
+/* ---------------------------------------------------------------------------
+ * NEXT-3, second half: folding a dedispersed time series into a pulse profile.
+ * Every result figure of the paper is a folded profile (Figs. 1, 8, 13, 14;
+ * P:L59) but the method is not described; reading R17
+ * (DESIGN.md): sample j is taken at t_j = t0 + j*dt, its pulse phase is the
+ * fractional part of t_j / period, it falls into bin floor(phase * n_bins)
+ * (clamped to n_bins - 1), a bin's value is the SUM of its samples and the
+ * number of samples per bin is returned beside it (profile = sum / count).
+ * The bin decision is taken in fp64.
+ * ------------------------------------------------------------------------- */
+void oracle_fold(const double *series, long long n, double t0_s, double dt_s, double period_s, int n_bins,
+                 double *sum /* [n_bins] */, long long *count /* [n_bins] */)
+{
+    for (int b = 0; b < n_bins; ++b) { sum[b] = 0.0; count[b] = 0; }
+    for (long long j = 0; j < n; ++j) {
+        double turns = (t0_s + (double)j * dt_s) / period_s;
+        double phase = turns - floor(turns);
+        int b = (int)(phase * (double)n_bins);
+        if (b > n_bins - 1) b = n_bins - 1;
+        sum[b] += series[j];
+        count[b] += 1;
+    }
+}

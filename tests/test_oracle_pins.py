@@ -557,3 +557,26 @@ def test_p17_band_sum_raises_the_pulse_above_a_single_channel():
     single = out[0, w.n_chan - 1]
     assert snr(aligned) > 4.0 * snr(single)           # sqrt(64) = 8 in the ideal case
     assert snr(aligned) > 3.0 * snr(unaligned)
+
+
+# ----------------------------------------------------------------------------- P18: folding (NEXT-3)
+def test_p18_fold_closed_forms_and_numpy_bincount():
+    """(a) a constant series folds to sum == count; (b) with dt = period/n_bins exactly, sample j falls in bin
+    j mod n_bins, so a comb of period n_bins puts everything in one bin; (c) an independent implementation
+    (numpy mod + bincount) gives the same bins and sums on random data with an awkward period."""
+    oracle.build()
+    s, n = oracle.fold(np.ones(1000), 0.0, 1.0, 64.0, 64)
+    assert np.array_equal(s, n.astype(float)) and n.sum() == 1000 and n.max() - n.min() <= 1
+    comb = np.zeros(64 * 20)
+    comb[5::64] = 3.0
+    s, n = oracle.fold(comb, 0.0, 0.25, 16.0, 64)           # 0.25 and 16 are exact in binary
+    assert s[5] == 60.0 and s.sum() == 60.0 and np.all(n == 20)
+    rng = np.random.default_rng(18)
+    x = rng.normal(size=50_000) + 10.0
+    t0, dt, P, nb = 0.00123, 64e-6, 5.0e-3 * 1.000137, 39
+    s, n = oracle.fold(x, t0, dt, P, nb)
+    t = t0 + np.arange(x.size) * dt
+    ph = t / P - np.floor(t / P)
+    b = np.minimum((ph * nb).astype(int), nb - 1)
+    assert np.array_equal(n, np.bincount(b, minlength=nb))
+    assert np.allclose(s, np.bincount(b, x, nb), rtol=1e-12)
