@@ -152,6 +152,16 @@ int dedisp_band_shifts(dedisp_plan_t plan, int d, long long* h_shift);
 int dedisp_band_sum(dedisp_plan_t plan, const float* d_out, long long out_stride, long long n_out, float* d_series,
                     long long series_stride, void* cuda_stream);
 
+/*
+ * Folding a dedispersed time series into a pulse profile (every result figure of the paper is one: Figs. 1, 8, 13, 14,
+ * P:L59; the method is not described - reading R17): sample j, taken at t0_s + j*dt_s, goes
+ * to phase bin floor(frac(t/period_s) * n_bins) (decided in fp64); a bin holds the SUM of its samples and their count.
+ *   d_series DEVICE float [n];  d_sum DEVICE float [n_bins] and d_count DEVICE unsigned [n_bins]: both zeroed by
+ *   the call, then filled (floating-point sums in an unspecified order).  1 <= n_bins <= 4096.  No plan needed.
+ */
+int dedisp_fold(const float* d_series, long long n, double t0_s, double dt_s, double period_s, int n_bins, float* d_sum,
+                unsigned int* d_count, void* cuda_stream);
+
 int dedisp_destroy(dedisp_plan_t plan);
 
 const char* dedisp_strerror(int code);

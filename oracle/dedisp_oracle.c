@@ -45,6 +45,7 @@
  *   R11 detection |v|^2 = re^2 + im^2; integration = plain sum of n_int samples.
  *   R12 no zero padding; output j covers input times head + j*n_int ...
  *   R16 sub-band alignment in whole output samples against the top channel (oracle_band_sum).
+ *   R17 folding: bin = floor(frac(t/period) * n_bins) in fp64, sums and counts (oracle_fold).
  */
 #include <complex.h>
 #include <math.h>

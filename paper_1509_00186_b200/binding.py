@@ -17,7 +17,7 @@ SYMBOLS = (
     "dedisp_framing", "dedisp_plan", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
     "dedisp_execute_add",
     "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_profile_enable",
-    "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_destroy",
+    "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_fold", "dedisp_destroy",
     "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
 )
 
@@ -61,6 +61,7 @@ def _load() -> C.CDLL:
     L.dedisp_band_samples.restype = ll
     L.dedisp_band_shifts.argtypes = [vp, C.c_int, C.POINTER(ll)]
     L.dedisp_band_sum.argtypes = [vp, vp, ll, ll, vp, ll, vp]
+    L.dedisp_fold.argtypes = [vp, ll, C.c_double, C.c_double, C.c_double, C.c_int, vp, vp, vp]
     L.dedisp_destroy.argtypes = [vp]
     L.dedisp_strerror.argtypes = [C.c_int]
     L.dedisp_strerror.restype = C.c_char_p
@@ -100,6 +101,18 @@ def dedisp_framing(n_chan: int, bw_hz: float, f_center_hz: float, dm: Sequence[f
 def dedisp_plan(n_chan: int, bw_hz: float, f_center_hz: float, dm: Sequence[float], n_fft: int, n_int: int,
                 taper: str = "none") -> "Plan":
     return Plan(n_chan, bw_hz, f_center_hz, dm, n_fft, n_int, taper)
+
+
+def dedisp_fold(d_series, t0_s: float, dt_s: float, period_s: float, n_bins: int, stream=None):
+    """Fold a 1-D CUDA float32 series at period_s: returns (sum per bin float32 [n_bins], count per bin int32 [n_bins])."""
+    import torch
+    assert d_series.is_cuda and d_series.dtype == torch.float32 and d_series.is_contiguous() and d_series.dim() == 1
+    s = torch.empty(n_bins, dtype=torch.float32, device=d_series.device)
+    n = torch.empty(n_bins, dtype=torch.int32, device=d_series.device)
+    st = torch.cuda.current_stream(d_series.device).cuda_stream if stream is None else stream
+    _check(_lib.dedisp_fold(d_series.data_ptr(), d_series.numel(), t0_s, dt_s, period_s, n_bins, s.data_ptr(),
+                            n.data_ptr(), st), "dedisp_fold")
+    return s, n
 
 
 class Plan:

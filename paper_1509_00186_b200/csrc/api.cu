@@ -282,6 +282,15 @@ extern "C" int dedisp_band_sum(dedisp_plan_t p, const float* d_out, long long ou
     return dedisp_launch_band_sum(p, d_out, out_stride, d_series, series_stride, n_ser, (cudaStream_t)cuda_stream);
 }
 
+extern "C" int dedisp_fold(const float* d_series, long long n, double t0_s, double dt_s, double period_s, int n_bins,
+                           float* d_sum, unsigned int* d_count, void* cuda_stream)
+{
+    if (!d_series || !d_sum || !d_count || n <= 0 || n_bins <= 0 || n_bins > 4096 || !(dt_s > 0.0) || !(period_s > 0.0) ||
+        !isfinite(t0_s))
+        return DEDISP_EINVAL;
+    return dedisp_launch_fold(d_series, n, t0_s, dt_s, period_s, n_bins, d_sum, d_count, (cudaStream_t)cuda_stream);
+}
+
 extern "C" int dedisp_destroy(dedisp_plan_t p)
 {
     if (!p) return DEDISP_EINVAL;

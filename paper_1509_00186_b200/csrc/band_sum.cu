@@ -43,7 +43,45 @@ __global__ void __launch_bounds__(TJ * SLICES) band_sum_kernel(const float* __re
         series[(size_t)d * series_stride + j] = (part[0][tx] + part[1][tx]) + (part[2][tx] + part[3][tx]);
 }
 
+// Folding at a trial period (reading R17): bin = floor(frac((t0 + j*dt)/P) * n_bins) decided in fp64 (as the oracle
+// does), sums and counts collected in a shared-memory histogram per CTA and merged with one atomic per bin and CTA.
+__global__ void __launch_bounds__(256) fold_kernel(const float* __restrict__ series, long long n, double t0, double dt,
+                                                   double period, int n_bins, float* __restrict__ sum,
+                                                   unsigned int* __restrict__ count)
+{
+    extern __shared__ float sh_sum[];                                        // [n_bins] sums, then [n_bins] counts
+    unsigned int* sh_cnt = reinterpret_cast<unsigned int*>(sh_sum + n_bins);
+    for (int b = threadIdx.x; b < n_bins; b += blockDim.x) { sh_sum[b] = 0.f; sh_cnt[b] = 0u; }
+    __syncthreads();
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+        // no FMA contraction: the bin must come out exactly as in plain IEEE fp64 arithmetic (the oracle's)
+        const double turns = __ddiv_rn(__dadd_rn(t0, __dmul_rn((double)j, dt)), period);
+        const double phase = __dadd_rn(turns, -floor(turns));
+        int b = (int)__dmul_rn(phase, (double)n_bins);
+        if (b > n_bins - 1) b = n_bins - 1;
+        atomicAdd(&sh_sum[b], __ldg(series + j));
+        atomicAdd(&sh_cnt[b], 1u);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < n_bins; b += blockDim.x) {
+        if (sh_cnt[b]) { atomicAdd(&sum[b], sh_sum[b]); atomicAdd(&count[b], sh_cnt[b]); }
+    }
+}
+
 }  // namespace
+
+int dedisp_launch_fold(const float* d_series, long long n, double t0, double dt, double period, int n_bins,
+                       float* d_sum, unsigned int* d_count, cudaStream_t st)
+{
+    DEDISP_CUDA_TRY(cudaMemsetAsync(d_sum, 0, sizeof(float) * n_bins, st));
+    DEDISP_CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(unsigned int) * n_bins, st));
+    long long grid = (n + 256 * 16 - 1) / (256 * 16);  // ~16 samples per thread
+    if (grid > 1184) grid = 1184;
+    if (grid < 1) grid = 1;
+    fold_kernel<<<(unsigned)grid, 256, sizeof(float) * 2 * n_bins, st>>>(d_series, n, t0, dt, period, n_bins, d_sum, d_count);
+    DEDISP_CUDA_TRY(cudaGetLastError());
+    return DEDISP_OK;
+}
 
 int dedisp_launch_band_sum(const dedisp_plan_s* p, const float* d_out, long long out_stride, float* d_series,
                            long long series_stride, long long n_series, cudaStream_t st)

@@ -87,5 +87,7 @@ long long dedisp_n_blocks(const dedisp_plan_s* p, long long n_samp);
 // band_sum.cu
 int dedisp_launch_band_sum(const dedisp_plan_s* p, const float* d_out, long long out_stride, float* d_series,
                            long long series_stride, long long n_series, cudaStream_t st);
+int dedisp_launch_fold(const float* d_series, long long n, double t0, double dt, double period, int n_bins,
+                       float* d_sum, unsigned int* d_count, cudaStream_t st);
 // stream.cu
 void dedisp_stream_free(dedisp_plan_s* p);
