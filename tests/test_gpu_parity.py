@@ -390,3 +390,14 @@ def test_execute_is_cuda_graph_capturable(dd, torch):
         g.replay()
         torch.cuda.synchronize()
         assert torch.equal(out, want2)
+
+
+def test_gpu_matches_the_frozen_oracle_case(dd, torch):
+    """The stored oracle output of tests/golden (fp64, written by a script that calls only oracle/) as a second, frozen
+    reference for the CUDA path: Hann taper, a positive and a negative DM, three blocks."""
+    from test_oracle_pins import load_frozen_case
+    mod, frozen = load_frozen_case()
+    cfg, x, _ = mod.compute()
+    with dd.dedisp_plan(cfg.n_chan, cfg.bw_hz, cfg.f_center_hz, cfg.dm, cfg.n_fft, cfg.n_int, cfg.taper) as plan:
+        got = run_gpu(torch, plan, x)
+        assert_parity(got, frozen, plan.L // plan.n_int)

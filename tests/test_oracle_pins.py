@@ -580,3 +580,25 @@ def test_p18_fold_closed_forms_and_numpy_bincount():
     b = np.minimum((ph * nb).astype(int), nb - 1)
     assert np.array_equal(n, np.bincount(b, minlength=nb))
     assert np.allclose(s, np.bincount(b, x, nb), rtol=1e-12)
+
+
+# ----------------------------------------------------------------------------- frozen oracle output
+def load_frozen_case():
+    import importlib.util
+    here = os.path.join(os.path.dirname(__file__), "golden")
+    spec = importlib.util.spec_from_file_location("make_oracle_golden", os.path.join(here, "make_oracle_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    vals = np.loadtxt(os.path.join(here, "oracle_small_case.txt"))
+    with open(os.path.join(here, "oracle_small_case.txt")) as fh:
+        shape = [int(v) for v in [l for l in fh if l.startswith("# shape")][0].split()[2:]]
+    return mod, vals.reshape(shape)
+
+
+def test_oracle_output_is_frozen():
+    """The oracle still produces the stored values (written by tests/golden/make_oracle_golden.py, which calls only
+    oracle/ and datagen/): its arithmetic has not drifted.  1e-12 relative leaves room for libm differences only."""
+    mod, frozen = load_frozen_case()
+    _, _, out = mod.compute()
+    assert out.shape == frozen.shape
+    assert np.abs(out / frozen - 1.0).max() < 1e-12
