@@ -11,9 +11,11 @@ Recipe per frequency channel c (independent Philox stream keyed (seed, c)):
   noise   n[t] = sigma * (g1 + i g2)                      sigma = 20 counts per component
   pulse   p[t] = a * sigma * gate(t) * (g3 + i g4)        amplitude-modulated noise, gate = 1 while
                                                           ((t/dv - delay_c) mod P) < W
-  ISM     p' = IFFT( FFT(p) * exp(-i*phi) )               ONE zero-padded whole-series transform
-          phi(f) = 2*pi*D*DM*[ 1/(f_c+f) - 1/f_c + f/f_c^2 ]   cold-plasma phase of PAPER.md Eq. 1
-                                                          minus its constant and linear terms
+  ISM     p' = IFFT( FFT(p) * exp(-i*phi) )               ONE zero-padded whole-series transform, H = exp(-i*phi)
+                                                          as PAPER.md P:L107 defines the ISM transfer function
+          phi(f) = -2*pi*D*DM*[ 1/(f_c+f) - 1/f_c + f/f_c^2 ]  cold-plasma phase of PAPER.md Eq. 1 (its dispersive
+                                                          part is -2*pi*D*DM/f) minus the constant and linear terms
+                                                          (P:L112): low frequencies arrive later
   record  re, im = clip(rint(n + p'), -127, 127) as int8, layout [t][chan][2]
 delay_c = D*DM*(1/f_c^2 - 1/f_top^2) is the inter-channel dispersion delay, kept so the band looks
 like a real observation (the hot path does not remove it).
@@ -89,9 +91,11 @@ def _next_pow2(n: int) -> int:
 
 
 def _ism_phase(dm: float, f_c: float, f: np.ndarray) -> np.ndarray:
-    """Cold-plasma propagation phase (radians) relative to the channel centre, with the constant and
-    the linear (pure delay) terms removed (Eq. 1-2)."""
-    return 2.0 * np.pi * D_HZ2_S * dm * (1.0 / (f_c + f) - 1.0 / f_c + f / (f_c * f_c))
+    """Cold-plasma propagation phase phi (radians) of PAPER.md Eq. 1 relative to the channel centre, with the constant
+    and the linear (pure delay) terms removed (Eq. 1-2).  Eq. 1's dispersive part is
+    -2 pi (L f_p^2 / 2c) / f = -2 pi D DM / f; the ISM transfer function is exp(-i phi), whose group delay
+    (1/2 pi) dphi/df = D DM / f^2 is the dispersion delay law of P:L39-41."""
+    return -2.0 * np.pi * D_HZ2_S * dm * (1.0 / (f_c + f) - 1.0 / f_c + f / (f_c * f_c))
 
 
 def _gen_channel(w: Workload, c: int, f_c: float, f_top: float, t0: int, n: int, clip: bool = True) -> np.ndarray:

@@ -9,9 +9,11 @@
  * (stage order of P:L139-145 Fig. 4):
  *   1. unpack   x[n] = (float)in[b*L+n][c].re + i*(float)in[b*L+n][c].im,  n in [0,N)      (R10)
  *   2. forward  S[k] = sum_n x[n] exp(-2*pi*i*k*n/N)
- *   3. chirp    Y[k] = S[k] * w(f_k) * exp(+2*pi*i*psi),  psi = D*DM_d*f_k^2/(f_c^2*(f_c+f_k)) (Eq. 3)
+ *   3. chirp    Y[k] = S[k] * w(f_k) * exp(-2*pi*i*psi),  psi = D*DM_d*f_k^2/(f_c^2*(f_c+f_k)):  the INVERSE
+ *               of the ISM's in-band term, which Eq. 3 prints as exp(+2*pi*i*psi); taper w; R1.
  *               D = 4.148808e15 Hz^2 s / (pc cm^-3), f_c = F - B/2 + (c+1/2)*B/C,
- *               f_k = k*dv/N (k < N/2) or (k-N)*dv/N, dv = B/C
+ *               f_k = k*dv/N (k < N/2) or (k-N)*dv/N, dv = B/C; baseband frequency rises with sky frequency.
+ *               DM_d > 0 removes the dispersion of a pulsar at that DM; DM_d < 0 applies Eq. 3 itself.
  *   4. inverse  y[n] = (1/N) sum_k Y[k] exp(+2*pi*i*k*n/N)                                    (R7)
  *   5. discard  keep n in [head, head+L), L = N - head - tail                                (R9)
  *   6. detect + integrate  out[d][c][b*L/n_int + j] = sum_{i<n_int} |y[head + j*n_int + i]|^2 (R11)
@@ -59,8 +61,9 @@ typedef struct {
 /*
  * Overlap-save framing (pure host arithmetic, no GPU needed).  P:L121/L145: the number of samples to discard is the
  * impulse-response length = dispersion time in the band.  R9: with the channel-centre reference the applied filter
- * delays the low edge (needs `head` past samples) and advances the high edge (needs `tail` future samples); one
- * framing for all channels and DMs:  head = roundup(n_del, n_int), head+tail = roundup(head+n_adv, lcm(32,n_int)).
+ * (DM > 0) holds the high band edge back by n_high samples (an output needs that much PAST input: `head`) and pulls
+ * the low edge forward by n_low samples (FUTURE input: `tail`); one framing for all channels and DMs:
+ * head = roundup(n_high, n_int), head+tail = roundup(head+n_low, lcm(32,n_int)).
  *   dm: HOST array [n_dm], pc cm^-3, negative allowed (conjugate chirp; head/tail roles swap).
  * Returns DEDISP_EINVAL if an argument is non-positive, F - B/2 <= 0, head+tail >= n_fft or L % n_int != 0.
  */

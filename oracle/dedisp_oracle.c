@@ -31,8 +31,13 @@
  * (see DESIGN.md "Oracle pins"); nothing is "parity unpinned".
  *
  * Readings of the paper (DESIGN.md "Readings" R1..R13) that this file fixes:
- *   R1  chirp sign: exp(+2*pi*i*psi) exactly as Eq. 3 prints it, applied to
- *       the output of a forward DFT with kernel exp(-2*pi*i*k*n/N).
+ *   R1  chirp sign: Eq. 3 (printed exp(+2*pi*i*psi)) is the ISM's own
+ *       in-band term -- the third term of Eq. 2 under H = exp(-i*phi), P:L107 --
+ *       and "the transfer function to correct for the dispersion within the
+ *       band is the inverse of the third term": the chirp applied is
+ *       exp(-2*pi*i*psi), to the output of a forward DFT with kernel
+ *       exp(-2*pi*i*k*n/N) of a band whose baseband frequency rises with sky
+ *       frequency.  A negative DM entry applies Eq. 3 itself.
  *   R2  reference frequency of psi = the channel centre f_c, f in [-dv/2, dv/2).
  *   R3  f_c = F - B/2 + (c + 1/2) * dv.
  *   R5  bin k of the N-point FFT is baseband frequency k*dv/N for k < N/2 and
@@ -187,7 +192,7 @@ double oracle_bin_freq(const oracle_cfg_t *cfg, int k)
 /* Chirp phase in CYCLES, Eq. 3 with f_o read as the channel centre
  * f_c (R2) and f_l as the offset f from it:
  *     psi = D * DM * f^2 / ((f + f_c) * f_c^2)
- * so that H = exp(i * 2*pi * psi). */
+ * so that Eq. 3 reads exp(i * 2*pi * psi) (the ISM term; its inverse is applied, R1). */
 double oracle_chirp_phase_cycles(double dm, double f_c_hz, double f_hz)
 {
     return ORACLE_D_HZ2_S * dm * f_hz * f_hz / ((f_hz + f_c_hz) * f_c_hz * f_c_hz);
@@ -201,9 +206,11 @@ double oracle_taper(int taper, double f_hz, double dv_hz)
     return 1.0;
 }
 
-/* The chirp function of one (DM, channel): H[k] = taper * exp(+2*pi*i*psi)
- * ("The taper function multiplied with the inverse transfer function
- * is known as the chirp function"; sign R1). */
+/* The chirp function of one (DM, channel): H[k] = taper * exp(-2*pi*i*psi),
+ * psi the phase of Eq. 3 in cycles (the correction "is the inverse of
+ * the third term in Equation 2", which Eq. 3 prints; "The taper
+ * function multiplied with the inverse transfer function is known as the
+ * chirp function"; sign R1). */
 void oracle_chirp(const oracle_cfg_t *cfg, int d, int c, double complex *H)
 {
     double dv = oracle_chan_width(cfg);
@@ -213,7 +220,7 @@ void oracle_chirp(const oracle_cfg_t *cfg, int d, int c, double complex *H)
         double psi = oracle_chirp_phase_cycles(cfg->dm[d], fc, f);
         psi -= floor(psi);                     /* reduce mod 1 cycle before trig */
         double ang = 2.0 * M_PI * psi;
-        H[k] = oracle_taper(cfg->taper, f, dv) * (cos(ang) + I * sin(ang));
+        H[k] = oracle_taper(cfg->taper, f, dv) * (cos(ang) - I * sin(ang));
     }
 }
 
@@ -225,14 +232,16 @@ static long long roundup_ll(long long x, long long m) { return ((x + m - 1) / m)
 static long long gcd_ll(long long a, long long b) { while (b) { long long t = a % b; a = b; b = t; } return a; }
 
 /* D = "the length of the impulse response" = dispersion time in the band
- * (P:L121).  With the channel-centre reference (R2) the applied filter
- * exp(+2*pi*i*psi) has group delay tau(f) = -dpsi/df = -D*DM*(1/f_c^2 - 1/(f_c+f)^2):
- * for DM > 0 the low band edge is delayed by
- *     t_del = D*DM*(1/(f_c - dv/2)^2 - 1/f_c^2)       (needs past samples: head)
- * and the high edge advanced by
- *     t_adv = D*DM*(1/f_c^2 - 1/(f_c + dv/2)^2)       (needs future samples: tail);
- * for DM < 0 the roles swap.  The worst case is the lowest channel.  One
- * framing for the whole plan:
+ * (P:L121).  With the channel-centre reference (R2) the ISM (Eq. 3)
+ * delays the low band edge against the centre by
+ *     t_lo = D*|DM|*(1/(f_c - dv/2)^2 - 1/f_c^2)
+ * and lets the high edge arrive early by
+ *     t_hi = D*|DM|*(1/f_c^2 - 1/(f_c + dv/2)^2)          (delay law).
+ * The applied filter exp(-2*pi*i*psi) has group delay +dpsi/df: for DM > 0 it
+ * holds the high edge back by t_hi (an output sample needs PAST input: head)
+ * and pulls the low edge forward by t_lo (needs FUTURE input: tail); for
+ * DM < 0 the roles swap.  The worst case is the lowest channel.  One framing
+ * for the whole plan:
  *     head  = roundup(n_head, n_int)
  *     D_tot = roundup(head + n_tail, lcm(32, n_int))
  *     tail  = D_tot - head,  L = N - D_tot
@@ -246,12 +255,12 @@ int oracle_framing(const oracle_cfg_t *cfg, int *head, int *tail, int *L)
         double lo = fc - 0.5 * dv, hi = fc + 0.5 * dv;
         for (int d = 0; d < cfg->n_dm; ++d) {
             double a = fabs(cfg->dm[d]);
-            double t_del = ORACLE_D_HZ2_S * a * (1.0 / (lo * lo) - 1.0 / (fc * fc));
-            double t_adv = ORACLE_D_HZ2_S * a * (1.0 / (fc * fc) - 1.0 / (hi * hi));
-            long long n_del = (long long)ceil(t_del * dv);
-            long long n_adv = (long long)ceil(t_adv * dv);
-            long long h = cfg->dm[d] >= 0.0 ? n_del : n_adv;
-            long long t = cfg->dm[d] >= 0.0 ? n_adv : n_del;
+            double t_lo = ORACLE_D_HZ2_S * a * (1.0 / (lo * lo) - 1.0 / (fc * fc));
+            double t_hi = ORACLE_D_HZ2_S * a * (1.0 / (fc * fc) - 1.0 / (hi * hi));
+            long long n_lo = (long long)ceil(t_lo * dv);
+            long long n_hi = (long long)ceil(t_hi * dv);
+            long long h = cfg->dm[d] >= 0.0 ? n_hi : n_lo;
+            long long t = cfg->dm[d] >= 0.0 ? n_lo : n_hi;
             if (h > need_head) need_head = h;
             if (t > need_tail) need_tail = t;
         }

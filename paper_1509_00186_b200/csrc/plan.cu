@@ -42,11 +42,14 @@ int dedisp_framing_impl(int n_chan, double bw, double F, const double* dm, int n
         for (int d = 0; d < n_dm; ++d) {
             if (!isfinite(dm[d])) return DEDISP_EINVAL;
             const double k = DEDISP_D_HZ2_S * fabs(dm[d]) * dv;        // seconds -> samples
-            const long long n_delay = (long long)ceil(k * (inv_lo - inv_c));  // low edge lags the centre
-            const long long n_adv = (long long)ceil(k * (inv_c - inv_hi));    // high edge leads it
+            // the ISM makes the low edge lag the channel centre and the high edge lead it (delay law P:L39-41); the
+            // correction (R1: the inverse of Eq. 3) holds the high edge back -- an output sample needs that much PAST
+            // input -- and pulls the low edge forward -- FUTURE input; a negative DM swaps the two
+            const long long n_low = (long long)ceil(k * (inv_lo - inv_c));
+            const long long n_high = (long long)ceil(k * (inv_c - inv_hi));
             const bool pos = dm[d] >= 0.0;
-            need_past = max_ll(need_past, pos ? n_delay : n_adv);
-            need_future = max_ll(need_future, pos ? n_adv : n_delay);
+            need_past = max_ll(need_past, pos ? n_high : n_low);
+            need_future = max_ll(need_future, pos ? n_low : n_high);
             smear = fmax(smear, k * (inv_lo - inv_hi));
         }
     }
@@ -71,7 +74,8 @@ extern "C" int dedisp_framing(int n_chan, double bw_hz, double f_center_hz, cons
 // ---------------------------------------------------------------------------------------------------------------
 // Plan-time tables, generated on the device with the phase in fp64
 // ---------------------------------------------------------------------------------------------------------------
-// chirp[d][c][k] = w(f_k) * exp(+2 pi i psi) / N,  psi = D DM f^2 / ((f + f_c) f_c^2) cycles (Eq. 3; R1, R2)
+// chirp[d][c][k] = w(f_k) * exp(-2 pi i psi) / N,  psi = D DM f^2 / ((f + f_c) f_c^2) cycles: the inverse of
+// the ISM's in-band term, which Eq. 3 prints as exp(+2 pi i psi); R1, R2
 __global__ void chirp_table_kernel(float2* __restrict__ chirp, const double* __restrict__ dm, int n_chan, int n_fft,
                                    double bw, double F, unsigned taper)
 {
@@ -94,7 +98,7 @@ __global__ void chirp_table_kernel(float2* __restrict__ chirp, const double* __r
         const double r = 2.0 * f / dv;
         w *= 1.0 - r * r;
     }
-    chirp[((size_t)d * n_chan + c) * n_fft + k] = make_float2((float)(w * co), (float)(w * s));
+    chirp[((size_t)d * n_chan + c) * n_fft + k] = make_float2((float)(w * co), (float)(-(w * s)));
 }
 
 __global__ void twiddle_table_kernel(float2* __restrict__ tw, int n_fft)

@@ -112,19 +112,19 @@ def test_p2_chirp_array_unit_modulus_sign_and_bin_order():
     assert oracle.bin_freq(cfg, 1023) == -dv / 1024
     # channel centres (R3): tile the band
     assert oracle.chan_freq(cfg, 0) == 317e6 + 125e3 and oracle.chan_freq(cfg, 63) == 333e6 - 125e3
-    # sign (R1): +i, i.e. angle(H[k]) = +2 pi psi for small psi
+    # sign (R1): the applied chirp is the INVERSE of Eq. 3, i.e. angle(H[k]) = -2 pi psi for small psi
     k = 3
     psi = float(mpmath.mpf(D_HZ) * 10 * mpmath.mpf(oracle.bin_freq(cfg, k)) ** 2
                 / ((oracle.chan_freq(cfg, 0) + oracle.bin_freq(cfg, k)) * oracle.chan_freq(cfg, 0) ** 2))
     assert 0 < psi < 0.25
-    assert abs(np.angle(H[k]) - 2 * np.pi * psi) < 1e-12
+    assert abs(np.angle(H[k]) + 2 * np.pi * psi) < 1e-12
     # independent full-array evaluation with mpmath at a few bins, including large phases
     mpmath.mp.dps = 40
     fc = mpmath.mpf(oracle.chan_freq(cfg, 0))
     for k in (100, 511, 512, 700, 1023):
         f = mpmath.mpf(oracle.bin_freq(cfg, k))
         ph = 2 * mpmath.pi * mpmath.mpf(D_HZ) * 10 * f ** 2 / ((fc + f) * fc ** 2)
-        ref = complex(mpmath.cos(ph), mpmath.sin(ph))
+        ref = complex(mpmath.cos(ph), -mpmath.sin(ph))
         assert abs(H[k] - ref) < 1e-11
 
 
@@ -157,12 +157,21 @@ def test_p3_group_delay_is_the_cold_plasma_delay():
     assert abs(oracle.smear_seconds(10.0, lo, hi) - 4.148808e-3 * 10 * ((lo / 1e9) ** -2 - (hi / 1e9) ** -2)) < 1e-15
 
 
-def test_p3_filter_delays_low_edge_advances_high_edge():
-    """Sign bookkeeping of R1/R9: tau(f) = -dpsi/df > 0 (delay) below centre, < 0 above, for DM > 0."""
+def test_p3_ism_term_delays_low_edge_and_the_applied_chirp_undoes_it():
+    """Sign bookkeeping of R1/R9.  Eq. 3 = exp(+2 pi i psi) is the ISM term: with H = exp(-i phi) its group
+    delay is (1/2 pi) dphi/df = -dpsi/df, > 0 (late) below the channel centre and < 0 (early) above it for DM > 0,
+    the low side the longer one (1/f^2 law).  The chirp the oracle applies has the opposite phase slope
+    (the inverse of the third term), bin by bin."""
     dm, fc, h = 10.0, 317.125e6, 1.0
     tau = lambda f: -(oracle.chirp_phase_cycles(dm, fc, f + h) - oracle.chirp_phase_cycles(dm, fc, f - h)) / (2 * h)
     assert tau(-100e3) > 0 and tau(+100e3) < 0
-    assert tau(-100e3) > -tau(+100e3)          # the low side is the longer one (1/f^2 law)
+    assert tau(-100e3) > -tau(+100e3)
+    cfg = cfg_tiny()
+    H = oracle.chirp(cfg, 0, 0)
+    fc0 = oracle.chan_freq(cfg, 0)
+    for k in (1, 2, 1022, 1023):                     # small phases: no unwrapping needed
+        psi = oracle.chirp_phase_cycles(10.0, fc0, oracle.bin_freq(cfg, k))
+        assert 0 < psi < 0.1 and abs(np.angle(H[k]) + 2 * np.pi * psi) < 1e-12
 
 
 # ----------------------------------------------------------------------------- P4: numbers the paper prints
@@ -247,6 +256,12 @@ def test_p5_framing_negative_dm_swaps_head_and_tail():
     b = oracle.framing(cfg_tiny(dm=(-10.0,), n_int=1))
     assert a[0] + a[1] == b[0] + b[1]
     assert a[0] > a[1] - 32 and b[0] <= a[1] and b[1] >= a[0]
+    # a case where the two sides differ clearly (2 MHz channel at 60 MHz): DM > 0 puts the SHORTER, high-edge side
+    # (375 samples) in head and the longer low-edge side (394) in tail; DM < 0 the other way round.  By hand:
+    # D*0.005*2e6*(1/60e6^2 - 1/61e6^2) = 374.7, D*0.005*2e6*(1/59e6^2 - 1/60e6^2) = 393.8
+    p = oracle.framing(oracle.OracleConfig(1, 2e6, 60e6, (0.005,), 2048, 1))
+    n = oracle.framing(oracle.OracleConfig(1, 2e6, 60e6, (-0.005,), 2048, 1))
+    assert p[0] == 375 and n[0] == 394 and p[0] + p[1] == n[0] + n[1] == 800 and p[1] >= 394 and n[1] >= 375
     with pytest.raises(ValueError):
         oracle.framing(cfg_tiny(dm=(100.0,)))       # smear 1626 samples > N = 1024
 
@@ -260,7 +275,8 @@ def _to_int8(z):
 
 
 def _whole_series_filter(x, dm, fc, dv, sign):
-    """ONE long transform over the whole series (numpy FFT): multiply by exp(sign * 2 pi i psi)."""
+    """ONE long transform over the whole series (numpy FFT): multiply by exp(sign * 2 pi i psi);
+    sign = +1 is Eq. 3 as printed, the ISM's dispersing term."""
     n = x.size
     f = np.fft.fftfreq(n, d=1.0 / dv)
     psi = D_HZ * dm * f * f / ((fc + f) * fc * fc)
@@ -334,7 +350,7 @@ def test_p8_nonzero_head_boxcar_with_dm_pair():
 @pytest.mark.parametrize("dm", [10.0, -10.0])
 def test_p9_dispersed_delta_collapses_to_a_delta(dm):
     """north_star identity: a delta pulse dispersed at DM collapses back to a delta when dedispersed at
-    the same DM.  The delta is dispersed with conj(H) through ONE whole-series numpy FFT (independent of
+    the same DM.  The delta is dispersed with Eq. 3 as printed through ONE whole-series numpy FFT (independent of
     the block framing), quantised to int8, then run through the block algorithm with n_int = 1.
     Deltas sit mid-block, at the last valid sample of block 0 and at the first valid sample of block 1:
     a wrong head/tail split or a wrong chirp sign smears or loses them."""
@@ -347,7 +363,7 @@ def test_p9_dispersed_delta_collapses_to_a_delta(dm):
     x = np.zeros(T, complex)
     for s in spots:
         x[s] = A
-    xd = _whole_series_filter(x, dm, fc, dv, sign=-1)           # disperse = conj of the applied chirp
+    xd = _whole_series_filter(x, dm, fc, dv, sign=+1)           # disperse = Eq. 3 = conj of the applied chirp
     assert np.max(np.abs(xd)) < 127
     out = oracle.dedisp(cfg, _to_int8(xd[:, None]))[0, 0]
     assert out.size == 3 * L
@@ -372,7 +388,7 @@ def test_p9_misplaced_discard_fails_visibly():
     T = 2 * L + head + tail
     x = np.zeros(T, complex)
     x[head] = 700.0                                           # first valid sample of block 0
-    xd = _whole_series_filter(x, 10.0, fc, dv, sign=-1)
+    xd = _whole_series_filter(x, 10.0, fc, dv, sign=+1)
     xi = _to_int8(xd[:, None])
     out, volt = oracle.dedisp_units(cfg, xi, [0], [0], want_voltage=True)
     assert abs(volt[0, 0, 0]) ** 2 / 700.0 ** 2 > 0.98
@@ -381,7 +397,7 @@ def test_p9_misplaced_discard_fails_visibly():
     # emulate "discard everything at the end": sample index 0 of a block needs `head` past samples that
     # the block does not contain -> the same delta placed at block-local index 0 does not collapse.
     x2 = np.zeros(T, complex); x2[0] = 700.0
-    xd2 = _whole_series_filter(x2, 10.0, fc, dv, sign=-1)
+    xd2 = _whole_series_filter(x2, 10.0, fc, dv, sign=+1)
     blk = np.fft.ifft(np.fft.fft(np.rint(xd2[:1024].real) + 1j * np.rint(xd2[:1024].imag)) * oracle.chirp(cfg, 0, 0))
     assert abs(blk[0]) ** 2 / 700.0 ** 2 < 0.9                # polluted by the circular wrap
 
@@ -419,7 +435,7 @@ def test_p12_bruteforce_time_domain_circular_convolution(n_fft):
             f = (k if k < n_fft // 2 else k - n_fft) * dv / n_fft
             ph = 2 * mpmath.pi * mpmath.mpf(D_HZ) * mpmath.mpf("0.02") * mpmath.mpf(f) ** 2 / (
                 (mpmath.mpf(fc) + f) * mpmath.mpf(fc) ** 2)
-            H[k] = complex(mpmath.cos(ph), mpmath.sin(ph))
+            H[k] = complex(mpmath.cos(ph), -mpmath.sin(ph))     # inverse of Eq. 3 (R1)
         h = np.array([sum(H[k] * np.exp(2j * np.pi * k * m / n_fft) for k in range(n_fft)) / n_fft
                       for m in range(n_fft)])
         ref = []
@@ -602,3 +618,96 @@ def test_oracle_output_is_frozen():
     _, _, out = mod.compute()
     assert out.shape == frozen.shape
     assert np.abs(out / frozen - 1.0).max() < 1e-12
+
+
+# ----------------------------------------------------------------------------- P19: physical sign pin (independent of Eq. 3)
+def _dispersed_band_impulse(C, B, F, dm, T, t0_s, A):
+    """A whole-band impulse that went through the ISM, built from the DELAY LAW alone (a component at
+    sky frequency f arrives D*DM/f^2 late), then split into C critically sampled channels by one FFT (an ideal
+    brick-wall channeliser; channel c covers [F-B/2 + c dv, F-B/2 + (c+1) dv), R3, baseband frequency rising with sky
+    frequency, R5).  The transfer function is exp(-i phi) with (1/2 pi) dphi/df = delay, delays measured
+    against the top band edge: phi(f) = -2 pi D DM (1/f + f/f_top^2).  Returns complex [T][C]."""
+    M = C * T
+    nu = np.fft.fftfreq(M, d=1.0 / B)                       # baseband frequency of the whole band, sky = F + nu
+    f_top = F + B / 2
+    X = A * np.exp(-2j * np.pi * nu * t0_s)                 # impulse at t0
+    X = X * np.exp(+2j * np.pi * D_HZ * dm * (1.0 / (F + nu) + nu / f_top ** 2))
+    Xs = np.fft.fftshift(X)                                 # ascending sky frequency
+    chans = [np.fft.ifft(np.fft.ifftshift(Xs[c * T:(c + 1) * T])) for c in range(C)]
+    return np.stack(chans, axis=1)
+
+
+def test_p19_physically_dispersed_band_impulse_collapses_with_one_positive_dm():
+    """The pin that ties the chirp sign (R1), the framing roles (R9) and the band alignment (R16) to physics rather
+    than to each other: an impulse dispersed by the delay law (no use of Eq. 3) must, with ONE plan at DM = +0.5,
+    (a) collapse inside every channel, (b) sit at the arrival time of the channel centre, and (c) line up in the band
+    sum.  The opposite DM sign must smear it further."""
+    C, B, F, dm, T, N = 8, 1e6, 100e6, 0.5, 4096, 256
+    dv = B / C
+    A = 800.0
+    t0 = 1500.25 / dv
+    z = _dispersed_band_impulse(C, B, F, dm, T, t0, A)
+    x = _to_int8(z)
+    cfg = oracle.OracleConfig(C, B, F, (dm,), N, 1)
+    head, tail, L = oracle.framing(cfg)
+    out = oracle.dedisp(cfg, x)[0]                                        # [C][n_out], n_int = 1
+    fcs = np.array([oracle.chan_freq(cfg, c) for c in range(C)])
+    arrive = (t0 + D_HZ * dm * (fcs ** -2.0 - (F + B / 2) ** -2.0)) * dv - head   # output sample index
+    undisp = np.abs(z) ** 2
+    for c in range(C):
+        pk = int(out[c].argmax())
+        assert abs(pk - arrive[c]) <= 1.0, (c, pk, arrive[c])             # (b)
+        frac = out[c, pk - 2: pk + 3].sum() / out[c].sum()
+        # (a) collapsed: a band-limited impulse half a sample off the grid keeps 2*(sinc^2(.5)+sinc^2(1.5))+sinc^2(2.5)
+        # = 0.916 of its energy in 5 samples, one on the grid keeps all of it; measured 0.921 ... 0.998
+        assert frac > 0.90, (c, frac)
+        assert out[c].max() > 6.0 * undisp[:, c].max()                    # ... from a smear of ~65 samples
+    s = oracle.band_sum(cfg, out[None])[0]                                # (c)
+    pk = int(s.argmax())
+    assert s[pk - 2: pk + 3].sum() > 0.90 * s.sum()
+    assert s.max() > 0.5 * C * A * A
+    # negative control: the opposite sign doubles the smear instead of removing it
+    cfg_n = oracle.OracleConfig(C, B, F, (-dm,), N, 1)
+    out_n = oracle.dedisp(cfg_n, x)[0]
+    for c in range(C):
+        assert out_n[c].max() < 0.6 * undisp[:, c].max() + 50.0
+
+
+# ----------------------------------------------------------------------------- P20: the sampled-unit and unpack entry points
+def test_p20_dedisp_units_equals_the_rows_of_dedisp():
+    """oracle.dedisp_units is the only reference of the full-size GPU tests: every (channel, block) unit of a 3-channel,
+    4-block, 3-DM case must equal the matching slice of oracle.dedisp exactly (same arithmetic, different indexing),
+    voltages included (their squared sums reproduce the intensities)."""
+    cfg = cfg_tiny(n_chan=3, bw_hz=0.75e6, f_center_hz=317.375e6, dm=(10.0, -6.0, 3.0), n_int=8)
+    head, tail, L = oracle.framing(cfg)
+    x = datagen.uniform_int8(4 * L + head + tail + 5, 3, seed=20)
+    full = oracle.dedisp(cfg, x)
+    per = L // cfg.n_int
+    assert full.shape == (3, 3, 4 * per)
+    chans = [c for c in range(3) for b in range(4)]
+    blocks = [b for c in range(3) for b in range(4)]
+    order = np.random.default_rng(20).permutation(len(chans))           # not in storage order
+    chans, blocks = np.asarray(chans)[order], np.asarray(blocks)[order]
+    units, volt = oracle.dedisp_units(cfg, x, chans, blocks, n_threads=3, want_voltage=True)
+    assert units.shape == (12, 3, per) and volt.shape == (12, 3, L)
+    for i, (c, b) in enumerate(zip(chans, blocks)):
+        for d in range(3):
+            assert np.array_equal(units[i, d], full[d, c, b * per:(b + 1) * per]), (i, c, b, d)
+            p = (np.abs(volt[i, d]) ** 2).reshape(per, cfg.n_int).sum(1)
+            assert np.allclose(p, units[i, d], rtol=1e-12, atol=0)
+    # the DM = +10 and DM = -6 rows really differ (a stride bug that repeats one DM would pass the loop above otherwise)
+    assert np.abs(units[:, 0] - units[:, 1]).max() > 1.0
+
+
+def test_p20_unpack_block_is_the_framed_slice_of_the_input():
+    cfg = cfg_tiny(n_chan=5, bw_hz=1.25e6, f_center_hz=317.625e6, n_int=4)
+    head, tail, L = oracle.framing(cfg)
+    x = datagen.uniform_int8(3 * L + head + tail, 5, seed=21)
+    nb = oracle.n_blocks(cfg, x.shape[0])
+    assert nb == 3
+    for c in (0, 2, 4):
+        for b in (0, nb - 1):
+            got = oracle.unpack_block(cfg, x, c, b)
+            assert got.dtype == np.float64 and got.shape == (cfg.n_fft, 2)
+            assert np.array_equal(got, x[b * L: b * L + cfg.n_fft, c, :].astype(np.float64))
+    assert (x == -128).any()
