@@ -35,11 +35,33 @@ if ROOT not in sys.path:
 
 METRIC = "complex Msamples/s dedispersed"
 UNIT = "Msamples/s"
-N_SM, FP32_LANES_PER_SM = 148, 128   # B200: 148 SMs x 4 sub-partitions x 32 FP32 lanes (guides: B300_MICROARCH)
+FP32_LANES_PER_SM = 128   # sm_100: 4 sub-partitions x 32 FP32 lanes per SM; the SM count is read from the device
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full`
-# capture (profiles/), keyed by workload; None until a capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"gmrt32": 1.0419e9 + 0.4826e9}   # profiles/r1h_ncu_gmrt32.md
+
+def ncu_traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel, from the committed summary of the
+    latest `ncu --set full` capture (profiles/ncu_traffic.csv: workload,kernel,dram_read_bytes,dram_write_bytes,capture).
+    ncu cannot run inside a timed bench, so this is NOT measured in this run: the line names its source, and it is None
+    when no capture of this workload is on file."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            for ln in f:
+                p = [v.strip() for v in ln.split(",")]
+                if len(p) >= 5 and p[0] == workload:
+                    return float(p[2]) + float(p[3]), f"profiles/ncu_traffic.csv ({p[4]}; not measured in this run)"
+    except Exception:
+        pass
+    return None, "no ncu capture of this workload on file"
+
+
+def stats(ms):
+    """best / median / mean / sigma of per-step times (the paper reports mean +- sigma of 1000 runs)."""
+    a = sorted(ms)
+    n = len(a)
+    mean = sum(a) / n
+    return {"best": a[0], "median": a[n // 2] if n % 2 else 0.5 * (a[n // 2 - 1] + a[n // 2]), "mean": mean,
+            "std": (sum((v - mean) ** 2 for v in a) / max(n - 1, 1)) ** 0.5, "n": n}
 
 
 def parse_args():
@@ -54,6 +76,8 @@ def parse_args():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT+elementwise reference point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the cpu_baseline leg")
+    ap.add_argument("--ubench", choices=("fp32-issue",), default=None,
+                    help="run a micro-benchmark instead of the bench (one JSON line; not the bench contract)")
     return ap.parse_args()
 
 
@@ -294,19 +318,20 @@ def run_ours(args):
     torch.cuda.synchronize()
     sampler = ClockSampler(local).start() if rank == 0 else None
     time.sleep(0.3)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     plan.profile_enable(True)
     barrier()
     torch.cuda.synchronize()
     mark0 = sampler.mark() if sampler else 0
-    ev0.record()
-    for _ in range(args.steps):
+    evs[0].record()
+    for i in range(args.steps):
         plan.execute(d_in, d_out)
-    ev1.record()
+        evs[i + 1].record()
     torch.cuda.synchronize()
     barrier()
     mark1 = sampler.mark() if sampler else 0
-    ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+    ms_total = max_over_ranks(evs[0].elapsed_time(evs[-1]))
+    step_stats = stats([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
     ms_ct, ms_fused, n_prof = plan.profile_read()
     plan.profile_enable(False)
     # keep the load on while the sampler catches at least a few readings (short runs finish between two samples)
@@ -343,22 +368,46 @@ def run_ours(args):
             assert e2e_step() == n_out
         barrier()
         torch.cuda.synchronize()
+        e2e_ms = []
         t0 = time.perf_counter()
         for _ in range(args.steps):
+            t1 = time.perf_counter()
             e2e_step()
+            e2e_ms.append((time.perf_counter() - t1) * 1e3)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         barrier()
         dt = max_over_ranks(dt) / args.steps
         plan.stream_end()
         same = bool(torch.equal(h_out, d_out.cpu()))
+        # the third roofline ("memory transfers turn out to be relatively expensive"): the box's own
+        # pinned copy rates, one plain cudaMemcpyAsync of the step's whole input / output through torch, same run
+        d_tmp = torch.empty_like(d_in)
+        c0, c1, c2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        d_tmp.copy_(h_in, non_blocking=True)
+        h_out.copy_(d_out, non_blocking=True)
+        torch.cuda.synchronize()
+        c0.record()
+        d_tmp.copy_(h_in, non_blocking=True)
+        c1.record()
+        h_out.copy_(d_out, non_blocking=True)
+        c2.record()
+        torch.cuda.synchronize()
+        h2d_gbs = h_in.numel() / (c0.elapsed_time(c1) * 1e-3) / 1e9
+        d2h_gbs = h_out.numel() * 4 / (c1.elapsed_time(c2) * 1e-3) / 1e9
+        del d_tmp
         e2e = {"value": world * samples / dt / 1e6, "unit": UNIT,
                "h2d_bytes_per_step": int(h_in.numel()), "d2h_bytes_per_step": int(h_out.numel() * 4),
                "ms_per_step": dt * 1e3, "real_time_factor": world * samples / dt / w.bw_hz,
                "chunk_samples": chunk, "chunks_per_step": (T + chunk - 1) // chunk,
                "timer": "host wall clock around all pushes + stream_sync",
                "api": "dedisp_stream_push (pinned host int8 in, pinned host fp32 out)",
-               "equals_device_resident_output": same}
+               "equals_device_resident_output": same, "ms_per_step_stats": stats(e2e_ms),
+               "pcie": {"bound": "pcie", "h2d_gbs_measured": h2d_gbs, "d2h_gbs_measured": d2h_gbs,
+                        "h2d_gbs_achieved": h_in.numel() / dt / 1e9,
+                        "frac_of_pcie": h_in.numel() / dt / 1e9 / h2d_gbs,
+                        "how": "one cudaMemcpyAsync of the step's whole pinned input (H2D) and output (D2H), CUDA "
+                               "events, same run; H2D is the longer direction and bounds the streamed step"}}
         del h_out
 
     # ---- cuFFT + elementwise chain on the same framing: a reference point, never part of the product --------------------
@@ -402,7 +451,9 @@ def run_ours(args):
     # ---- roofline of the dominant (fused) kernel --------------------------------------------------------------------
     peaks, peaks_src = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    N_SM = torch.cuda.get_device_properties(local).multi_processor_count
     fp32_peak_tf = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    traffic, traffic_source = ncu_traffic(w.name)
     fused_ms = ms_fused / max(n_prof, 1)
     ct_ms = ms_ct / max(n_prof, 1)
     flops = n_units * nominal_flops_per_unit(w.n_fft, L, plan.n_dm)
@@ -410,7 +461,7 @@ def run_ours(args):
     achieved_tf = flops / (fused_ms * 1e-3) / 1e12
     roofline = {
         "bound": "alu", "kernel": "fused_aos_kernel", "achieved": achieved_tf, "peak": fp32_peak_tf,
-        "unit": "TFLOP/s", "frac": achieved_tf / fp32_peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+        "unit": "TFLOP/s", "frac": achieved_tf / fp32_peak_tf, "traffic": traffic, "traffic_source": traffic_source,
         "peak_source": f"{N_SM} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 (FMA) x {sm_max:.0f} MHz "
                        f"(sm_max_mhz of MEASURED_PEAKS.json, {peaks_src})",
         "flops_per_launch": flops, "ms_per_launch": fused_ms, "share_of_step": fused_ms / ms_step,
@@ -446,7 +497,8 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "ms_per_step": ms_step, "ms_per_step_stats": step_stats, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "real_time_factor": value * 1e6 / w.bw_hz,
         "config": {"workload": w.name, "n_chan": w.n_chan, "bw_hz": w.bw_hz, "f_center_hz": w.f_center_hz,
@@ -467,9 +519,28 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_ubench(args):
+    """--ubench fp32-issue: SM sub-partition cycles per radix-2 butterfly for every instruction form of
+    dedisp_ubench_fp32 (csrc/ubench.cu); the numbers DESIGN.md section 6 quotes come from this command."""
+    import torch
+    import paper_1509_00186_b200 as dd
+    torch.cuda.set_device(0)
+    sampler = ClockSampler(0).start()
+    time.sleep(0.3)
+    rows = []
+    for form, name in enumerate(dd.UBENCH_FORMS):
+        best = min(dd.dedisp_ubench_fp32(form, 8192) for _ in range(3))
+        rows.append({"form": form, "what": name, "cycles_per_butterfly": best[0], "ms": best[1]})
+    clocks = sampler.stop()
+    print(json.dumps({"ubench": "fp32-issue", "unit": "SM sub-partition cycles per butterfly (8 warps per sub-partition)",
+                      "rows": rows, "clocks": clocks}), flush=True)
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.ubench:
+        run_ubench(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

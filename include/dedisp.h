@@ -165,6 +165,20 @@ int dedisp_band_sum(dedisp_plan_t plan, const float* d_out, long long out_stride
 int dedisp_fold(const float* d_series, long long n, double t0_s, double dt_s, double period_s, int n_bins, float* d_sum,
                 unsigned int* d_count, void* cuda_stream);
 
+/*
+ * FP32 issue-rate micro-benchmark of the packed f32x2 instruction forms the fused kernel is built from (measurement
+ * support for the "alu" roofline of DESIGN.md section 6; `python bench.py --ubench fp32-issue`).  Runs one persistent
+ * 1024-thread CTA per SM (64 registers per thread, 8 warps per SM sub-partition, 8 independent complex pairs per
+ * thread) for `iters` iterations of radix-2 butterfly form `form` and returns the SM sub-partition cycles per
+ * butterfly (clock64, mean over SMs) and the CUDA-event time of the launch.  Forms: 0 plain (2 FADD2); 1 with +-i
+ * (2 FADD2, lane-swapped operand); 2 general twiddle, conventional (FMUL2 + FFMA2 + 2 FADD2); 3 general twiddle
+ * folded into the butterfly (3 FFMA2, v = 2a - u); 4 form 3 with the twiddle rotated by i; 5 folded without the
+ * 2a - u step (4 FFMA2); 6 form 3 with an immediate twiddle; 7 form 2 with an immediate twiddle.
+ * Allocates and frees its own small device buffers; synchronises the device.  Errors: EINVAL, ENOMEM, ECUDA.
+ */
+#define DEDISP_UBENCH_FORMS 8
+int dedisp_ubench_fp32(int form, int iters, double* cycles_per_butterfly, double* ms);
+
 int dedisp_destroy(dedisp_plan_t plan);
 
 const char* dedisp_strerror(int code);
@@ -172,7 +186,9 @@ int dedisp_last_cuda_error(void); /* cudaError_t of the last DEDISP_ECUDA on thi
 
 /*
  * Test hooks (used by the parity tests only).
- * dedisp_debug_unpack: the framed, unpacked block (step 1) of (chan, block) as float [n_fft][2] on the DEVICE.
+ * dedisp_debug_unpack: the framed, unpacked block (step 1) of (chan, block) as float [n_fft][2] on the DEVICE: the
+ *                      values the fused kernel itself holds in registers after its int8 -> fp32 conversion (the
+ *                      corner turn and the kernel's own unpack run; the kernel stores and stops before the transform).
  * dedisp_debug_chirp:  copies the chirp table row (d, chan) to HOST as float [n_fft][2] (includes the 1/n_fft scale).
  * dedisp_debug_voltage: steps 1-5 for one (chan, block): DEVICE float [n_dm][L][2] dedispersed complex voltages.
  */

@@ -19,6 +19,7 @@ SYMBOLS = (
     "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_profile_enable",
     "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_fold", "dedisp_destroy",
     "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
+    "dedisp_ubench_fp32",
 )
 
 
@@ -63,6 +64,7 @@ def _load() -> C.CDLL:
     L.dedisp_band_sum.argtypes = [vp, vp, ll, ll, vp, ll, vp]
     L.dedisp_fold.argtypes = [vp, ll, C.c_double, C.c_double, C.c_double, C.c_int, vp, vp, vp]
     L.dedisp_destroy.argtypes = [vp]
+    L.dedisp_ubench_fp32.argtypes = [C.c_int, C.c_int, dp, dp]
     L.dedisp_strerror.argtypes = [C.c_int]
     L.dedisp_strerror.restype = C.c_char_p
     L.dedisp_last_cuda_error.argtypes = []
@@ -101,6 +103,18 @@ def dedisp_framing(n_chan: int, bw_hz: float, f_center_hz: float, dm: Sequence[f
 def dedisp_plan(n_chan: int, bw_hz: float, f_center_hz: float, dm: Sequence[float], n_fft: int, n_int: int,
                 taper: str = "none") -> "Plan":
     return Plan(n_chan, bw_hz, f_center_hz, dm, n_fft, n_int, taper)
+
+
+UBENCH_FORMS = ("plain 2xFADD2", "times-i 2xFADD2 (lane-swapped operand)", "twiddle conventional FMUL2+FFMA2+2xFADD2",
+                "twiddle folded 3xFFMA2 (v=2a-u)", "twiddle folded, rotated by i", "twiddle folded 4xFFMA2",
+                "immediate twiddle folded 3xFFMA2", "immediate twiddle conventional")
+
+
+def dedisp_ubench_fp32(form: int, iters: int = 4096):
+    """(SM sub-partition cycles per butterfly, ms of the launch) for instruction form `form` (see dedisp.h)."""
+    cyc, ms = C.c_double(), C.c_double()
+    _check(_lib.dedisp_ubench_fp32(form, iters, C.byref(cyc), C.byref(ms)), "dedisp_ubench_fp32")
+    return cyc.value, ms.value
 
 
 def dedisp_fold(d_series, t0_s: float, dt_s: float, period_s: float, n_bins: int, stream=None):

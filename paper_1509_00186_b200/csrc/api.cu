@@ -330,7 +330,7 @@ extern "C" int dedisp_debug_unpack(dedisp_plan_t p, const int8_t* d_in, long lon
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = debug_prepare(p, d_in, n_samp, chan, block, st);
     if (rc != DEDISP_OK) return rc;
-    return dedisp_launch_debug_unpack(p, p->d_xt, p->xt_cap_samp, chan, block, d_block, st);
+    return dedisp_launch_aos_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_block, 1, st);
 }
 
 extern "C" int dedisp_debug_voltage(dedisp_plan_t p, const int8_t* d_in, long long n_samp, int chan, long long block,
@@ -340,5 +340,5 @@ extern "C" int dedisp_debug_voltage(dedisp_plan_t p, const int8_t* d_in, long lo
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = debug_prepare(p, d_in, n_samp, chan, block, st);
     if (rc != DEDISP_OK) return rc;
-    return dedisp_launch_aos_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, st);
+    return dedisp_launch_aos_debug_voltage(p, p->d_xt, p->xt_cap_samp, chan, block, d_volt, 0, st);
 }

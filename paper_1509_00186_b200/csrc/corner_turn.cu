@@ -88,26 +88,7 @@ __global__ void __launch_bounds__(256) corner_turn_scalar_kernel(const int8_t* _
     }
 }
 
-// test hook: the framed block (chan, rows row0 .. row0+n_fft-1) of the channel-major scratch as fp32 (re, im)
-__global__ void debug_unpack_kernel(const int8_t* __restrict__ xt, long long xt_stride, int chan, long long row0,
-                                    int n_fft, float2* __restrict__ dst)
-{
-    const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= n_fft) return;
-    const int8_t* p = xt + ((long long)chan * xt_stride + row0 + n) * 2;
-    dst[n] = make_float2((float)p[0], (float)p[1]);
-}
-
 }  // namespace
-
-int dedisp_launch_debug_unpack(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
-                               long long block, float* d_block, cudaStream_t st)
-{
-    debug_unpack_kernel<<<(p->n_fft + 255) / 256, 256, 0, st>>>(d_xt, xt_stride, chan, block * p->L, p->n_fft,
-                                                                reinterpret_cast<float2*>(d_block));
-    DEDISP_CUDA_TRY(cudaGetLastError());
-    return DEDISP_OK;
-}
 
 int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int8_t* d_xt, long long xt_stride,
                               long long dst_t0, cudaStream_t st)

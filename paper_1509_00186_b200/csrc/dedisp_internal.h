@@ -65,14 +65,13 @@ int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, 
 // accumulate != 0: add to d_out instead of overwriting it
 int dedisp_launch_aos(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, long long nb, float* d_out,
                       long long out_stride, long long out_col0, int accumulate, cudaStream_t st);
+// debug: dump_unpack = 0 -> [n_dm][L] dedispersed voltages of (chan, block); 1 -> the [N] values the fused kernel holds
+// in registers right after its own int8 -> fp32 conversion
 int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
-                                    long long block, float* d_volt, cudaStream_t st);
+                                    long long block, float* d_volt, int dump_unpack, cudaStream_t st);
 int dedisp_aos_supported(int n_fft);
 size_t dedisp_aos_spec_bytes(int n_fft);  // valid after dedisp_aos_init()
 int dedisp_aos_init(void);                // sets the dynamic shared memory attributes once per process
-// corner_turn.cu: test hook
-int dedisp_launch_debug_unpack(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
-                               long long block, float* d_block, cudaStream_t st);
 // plan-time table generation on the device (fp64 phase)
 int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaStream_t st);
 int dedisp_launch_twiddle_table(const dedisp_plan_s* p, cudaStream_t st);

@@ -48,6 +48,7 @@ struct AosArgs {
     float2* spec;          // [gridDim.x][4U][N] forward-spectrum stash, used when n_dm > 1
     float2* volt;          // debug: [n_dm][L] voltages of block volt_block, else nullptr
     int volt_block;
+    int dump_unpack;       // debug (with volt != nullptr): store the registers right after unpack_int8x2 as [N] (re, im)
     int nb;                // blocks per channel
     int spc;               // super-items per channel = ceil(nb / 4U)
     int n_super;           // super-items to process
@@ -154,6 +155,13 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
         C x[16];
 #pragma unroll
         for (int m = 0; m < 16; ++m) x[m] = unpack_int8x2(live ? (uint32_t)stage[t + m * TPU] : 0u);
+        if (a.volt && a.dump_unpack) {  // debug hook (one super-item): what the transform is about to see, bit for bit
+            if (live && a.volt_block == b) {
+#pragma unroll
+                for (int m = 0; m < 16; ++m) a.volt[t + m * TPU] = x[m];
+            }
+            return;  // uniform over the CTA; no cp.async is in flight (the prefetch is issued inside the transform)
+        }
 
         // 2. forward FFT; once every thread of the group is past the unpack, the staging buffer is
         //    free for the next super-item's rows
@@ -354,7 +362,7 @@ int dedisp_launch_aos(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_s
 }
 
 int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, long long xt_stride, int chan,
-                                    long long block, float* d_volt, cudaStream_t st)
+                                    long long block, float* d_volt, int dump_unpack, cudaStream_t st)
 {
     // the one super-item that holds (chan, block); blocks-per-channel = block + 1 is enough to address it
     AosArgs a;
@@ -364,5 +372,6 @@ int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, 
     a.n_super = 1;
     a.volt = reinterpret_cast<float2*>(d_volt);
     a.volt_block = (int)block;
+    a.dump_unpack = dump_unpack;
     return dispatch(p, a, st);
 }

@@ -1,9 +1,12 @@
 """GPU parity at BASELINE.json's FULL sizes (all five configs), in the launch configuration bench.py times
-(dedisp_execute on the whole device-resident workload).  The oracle cannot redo a whole config in seconds, so it
-recomputes SAMPLED (channel, block) units one by one: the first and last block of the lowest, a middle and the highest
-channel (the edges of the framing and of the grid) plus seeded random units; every sampled unit is compared element by
-element with BASELINE.json's tolerances.  Properties that hold at any size are checked on the whole output: every value
-finite and positive, and the mean level: noise floor n_int * (2 sigma^2 + 1/6) (P7) plus the pulsar's duty-cycle power."""
+(dedisp_execute on the whole device-resident workload).
+
+tiny, gmrt16, gmrt32, lowfreq: the WHOLE output is compared with the oracle, every (dm, channel, block) output block
+against BASELINE.json's tolerances (the oracle redoes gmrt32 in a few seconds on the box's cores; it is called through
+oracle.dedisp_units on 32 channels at a time to bound host memory -- that entry point is pinned to oracle.dedisp by P20).
+wideband (264 192 units of nine 16384-point transforms): every channel's first and last block plus seeded random units,
+> 1.5 % of the units.  Properties that hold at any size are checked on the whole output of every config: every value
+finite and positive, and the mean level = noise floor n_int * (2 sigma^2 + 1/6) (P7) plus the pulsar's duty-cycle power."""
 import os
 
 import numpy as np
@@ -31,8 +34,58 @@ def sampled_units(n_chan, nb, n_random, seed):
     return np.asarray(chans, dtype=np.int32), np.asarray(blocks, dtype=np.int64)
 
 
+def compare_units(d_out, ref, chans, blocks, per):
+    """ref [n_units][n_dm][per] (oracle) against the matching slices of d_out [n_dm][C][n_out] (device): worst block
+    relative L2 and worst max|d| / block RMS."""
+    import torch
+    idx = torch.from_numpy(blocks[:, None] * per + np.arange(per)[None, :]).cuda()             # [n_units][per]
+    got = d_out[:, torch.from_numpy(chans.astype(np.int64)).cuda()[:, None], idx]              # [n_dm][n_units][per]
+    got = got.permute(1, 0, 2).double().cpu().numpy()
+    den = (ref ** 2).sum(-1)
+    rel = np.sqrt(((got - ref) ** 2).sum(-1) / den)
+    mx = np.abs(got - ref).max(-1) / np.sqrt(den / per)
+    return float(rel.max()), float(mx.max())
+
+
+@pytest.mark.parametrize("name", ["tiny", "gmrt16", "gmrt32", "lowfreq"])
+def test_full_size_config_whole_output_parity(name):
+    """Every output block of the whole config against the oracle (a defect confined to particular CTAs or
+    super-item boundaries at full grid size would miss a 0.05 % sample)."""
+    import torch
+    import paper_1509_00186_b200 as dd
+    w = datagen.WORKLOADS[name]
+    x = datagen.generate(w)
+    cfg = oracle.OracleConfig(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
+    with dd.dedisp_plan(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int) as plan:
+        assert (plan.head, plan.tail, plan.L) == oracle.framing(cfg)
+        nb = plan.n_blocks(w.n_samp)
+        per = plan.L // plan.n_int
+        d_out = plan.execute(torch.from_numpy(x).cuda())
+        torch.cuda.synchronize()
+        assert d_out.shape == (plan.n_dm, w.n_chan, nb * per)
+        worst_rel = worst_mx = 0.0
+        step = 32
+        for c0 in range(0, w.n_chan, step):
+            cs = np.arange(c0, min(c0 + step, w.n_chan), dtype=np.int32)
+            chans = np.repeat(cs, nb)
+            blocks = np.tile(np.arange(nb, dtype=np.int64), cs.size)
+            ref = oracle.dedisp_units(cfg, x, chans, blocks, n_threads=NT)
+            rel, mx = compare_units(d_out, ref, chans, blocks, per)
+            worst_rel, worst_mx = max(worst_rel, rel), max(worst_mx, mx)
+            assert rel <= REL_L2_TOL and mx <= MAX_ABS_TOL, (name, c0, rel, mx)
+    print(f"{name}: all {w.n_chan * nb} units x {plan.n_dm} DMs, worst rel-L2 {worst_rel:.2e}, worst max/rms {worst_mx:.2e}")
+
+
+def wideband_units(n_chan, nb, n_random, seed):
+    """every channel's first and last block (the framing edges of every chirp row) + seeded random units"""
+    rng = np.random.default_rng(seed)
+    chans = np.concatenate([np.arange(n_chan), np.arange(n_chan), rng.integers(0, n_chan, n_random)])
+    blocks = np.concatenate([np.zeros(n_chan, np.int64), np.full(n_chan, nb - 1, np.int64), rng.integers(0, nb, n_random)])
+    return chans.astype(np.int32), blocks.astype(np.int64)
+
+
 @pytest.mark.parametrize("name,n_random", [("tiny", 40), ("gmrt16", 56), ("gmrt32", 56), ("lowfreq", 24),
-                                           ("wideband", 8)])
+                                           ("wideband", 512)])
 def test_full_size_config_sampled_parity(name, n_random):
     import torch
     import paper_1509_00186_b200 as dd
@@ -56,15 +109,18 @@ def test_full_size_config_sampled_parity(name, n_random):
         expect = 1.0 + (w.pulse_width_s / w.pulse_period_s) * w.pulse_amp_sigma ** 2
         assert abs(level / expect - 1.0) < 0.03, (level, expect)
         # sampled units against the oracle
-        chans, blocks = sampled_units(w.n_chan, nb, n_random, seed=w.seed + 100)
-        ref = oracle.dedisp_units(cfg, x, chans, blocks, n_threads=NT)          # [n_units][n_dm][per]
-        idx = torch.from_numpy(blocks[:, None] * per + np.arange(per)[None, :]).cuda()       # [n_units][per]
-        got = d_out[:, torch.from_numpy(chans.astype(np.int64)).cuda()[:, None], idx]        # [n_dm][n_units][per]
-        got = got.permute(1, 0, 2).double().cpu().numpy()
-    den = (ref ** 2).sum(-1)
-    rel = np.sqrt(((got - ref) ** 2).sum(-1) / den)
-    mx = np.abs(got - ref).max(-1) / np.sqrt(den / per)
-    assert rel.max() <= REL_L2_TOL, (name, float(rel.max()))
-    assert mx.max() <= MAX_ABS_TOL, (name, float(mx.max()))
-    print(f"{name}: {len(chans)} units x {plan.n_dm} DMs, worst rel-L2 {rel.max():.2e}, worst max/rms {mx.max():.2e}, "
+        if name == "wideband":
+            chans, blocks = wideband_units(w.n_chan, nb, n_random, seed=w.seed + 100)
+            assert len(chans) >= 0.015 * w.n_chan * nb
+        else:
+            chans, blocks = sampled_units(w.n_chan, nb, n_random, seed=w.seed + 100)
+        rel = mx = 0.0
+        for i0 in range(0, len(chans), 1024):                                   # bounded host memory per oracle call
+            sl = slice(i0, i0 + 1024)
+            ref = oracle.dedisp_units(cfg, x, chans[sl], blocks[sl], n_threads=NT)   # [n_units][n_dm][per]
+            r, m = compare_units(d_out, ref, chans[sl], blocks[sl], per)
+            rel, mx = max(rel, r), max(mx, m)
+    assert rel <= REL_L2_TOL, (name, rel)
+    assert mx <= MAX_ABS_TOL, (name, mx)
+    print(f"{name}: {len(chans)} units x {plan.n_dm} DMs, worst rel-L2 {rel:.2e}, worst max/rms {mx:.2e}, "
           f"level {level:.4f}")

@@ -107,11 +107,46 @@ def test_unpack_bit_exact_all_byte_values(dd, torch, n_chan, n_samp):
         xd = torch.from_numpy(x).cuda()
         nb = plan.n_blocks(n_samp)
         assert nb == oracle.n_blocks(cfg, n_samp) and nb >= 2
+        # dedisp_debug_unpack stores the registers of the FUSED kernel right after its own PRMT/FADD2 conversion
         for c in sorted({0, 1, n_chan // 2, n_chan - 1}):
-            for b in (0, nb - 1):
+            for b in range(nb):
                 got = plan.debug_unpack(xd, c, b).cpu().numpy()
                 ref = oracle.unpack_block(cfg, x, c, b)
                 assert np.array_equal(got.astype(np.float64), ref), (c, b)
+        got = plan.debug_unpack(xd, 0, 0).cpu().numpy()
+        assert np.array_equal(got[:256, 0], np.arange(-128, 128, dtype=np.float32))   # -128 ... 127 at known places
+
+
+@pytest.mark.parametrize("n_fft", [1024, 2048, 4096, 8192, 16384])
+def test_fused_kernel_unpack_bit_exact_every_size(dd, torch, n_fft):
+    """The same hook for every built transform size (each has its own staging geometry), on input that holds all 256
+    byte values in both components."""
+    n_chan = 8
+    dm = (1.0,)
+    cfg = oracle.OracleConfig(n_chan, 62.5e3 * n_chan, 325e6, dm, n_fft, 4)
+    head, tail, L = oracle.framing(cfg)
+    n_samp = 5 * L + head + tail + 3
+    x = datagen.uniform_int8(n_samp, n_chan, seed=n_fft)
+    with dd.dedisp_plan(n_chan, cfg.bw_hz, 325e6, dm, n_fft, 4) as plan:
+        xd = torch.from_numpy(x).cuda()
+        for c in (0, 3, 7):
+            for b in range(5):
+                got = plan.debug_unpack(xd, c, b).cpu().numpy()
+                assert np.array_equal(got.astype(np.float64), oracle.unpack_block(cfg, x, c, b)), (c, b)
+
+
+@pytest.mark.parametrize("n_fft,n_int,dm", [(1024, 4, (10.0,)), (4096, 4, (71.0, -20.0)), (16384, 32, (150.0,))])
+def test_full_range_int8_input_through_the_chirp(dd, torch, n_fft, n_int, dm):
+    """Uniform int8 input (every byte value, -128 included) through the whole path at a non-zero DM: the squares of a
+    DM = 0 run cannot tell -128 from +128, the dedispersed voltages can."""
+    n_chan = 6
+    cfg = oracle.OracleConfig(n_chan, 62.5e3 * n_chan, 325e6 if n_fft < 16384 else 150e6, dm, n_fft, n_int)
+    head, tail, L = oracle.framing(cfg)
+    x = datagen.uniform_int8(3 * L + head + tail + 11, n_chan, seed=7 * n_fft)
+    assert (x == -128).sum() > 100
+    ref = oracle.dedisp(cfg, x, n_threads=NT)
+    with dd.dedisp_plan(n_chan, cfg.bw_hz, cfg.f_center_hz, dm, n_fft, n_int) as plan:
+        assert_parity(run_gpu(torch, plan, x), ref, L // n_int)
 
 
 def test_dm_zero_is_integer_boxcar_power(dd, torch):
