@@ -28,131 +28,135 @@ __device__ __forceinline__ C crot(C a, float c, float s)
 }
 __device__ __forceinline__ C cmul(C a, C w) { return crot(a, w.x, w.y); }
 
-// d * exp(SIGN * 2*pi*i * j/16), j in [0, 8); j and SIGN are compile-time constants after unrolling.
+// ---------------------------------------------------------------------------------------------------------------
+// Radix-R pass = decimation-in-TIME butterflies with the pass's input twiddles folded in.
+//
+// A pass transforms y[r] = w^r x[r], r < R (w = the Stockham twiddle of this thread and pass; w = 1 in the first pass):
+// X[k] = sum_r y[r] W^{rk}, W = exp(SIGN 2 pi i / R).  With G_{M,o}[k] = (the M-point DFT of y[o + (R/M) j], j < M) / w^o
+//      G_{2M,o}[k]     = G_{M,o}[k] + T G_{M,o+s'}[k]
+//      G_{2M,o}[k + M] = G_{M,o}[k] - T G_{M,o+s'}[k],      T = w^{s'} W_{2M}^k,  s' = R/(2M),  o < s',  k < M
+// and X = G_{R,0}: the powers w^r never multiply the data on their own, every butterfly is u = a + T b, v = a - T b
+//      t = b * (c, c) + a;   u = (i b) * (s, s) + t;   v = a * 2 - u            (3 FFMA2, T = c + i s)
+// instead of FMUL2 + FFMA2 + 2 FADD2, and a pass needs only log2(R) powers of w and R/2 - 1 products with constants:
+// T for k >= M/2 is (SIGN i) T_{k - M/2}, an operand swizzle.  Measured per butterfly (bench.py --ubench fp32-issue):
+// 8.3 against 9.9 SM sub-partition cycles.  In the first pass T is a compile-time constant; 1 and +-i cost two FADD2.
+// ---------------------------------------------------------------------------------------------------------------
+
+// index of T = w^{R/M2} W_{M2}^{kb}, kb < max(1, M2/4), in a pass's twiddle set: M2 = 2, 4, 8, 16 -> 0, 1, 2..3, 4..7
+__host__ __device__ constexpr int tw_index(int M2, int kb) { return (M2 >= 4 ? M2 / 4 : 0) + kb; }
+template <int R> struct TwSet { C t[16 / R][R / 2]; };  // [sub-butterfly q][tw_index]; R/2 = 1 + 1 + 2 + 4 ... entries
+template <> struct TwSet<1> {};
+
+// (cos, SIGN sin) of 2 pi kb / M2 for the constants a radix <= 16 pass needs (kb < M2/4, so M2 = 8: kb = 1; 16: 1..3)
 template <int SIGN>
-__device__ __forceinline__ C mul_w16(C d, int j)
+__device__ __forceinline__ C w_const(int M2, int kb)
 {
     constexpr float s = (float)SIGN;
     constexpr float C1 = 0.92387953251128674f;  // cos(pi/8)
     constexpr float S1 = 0.38268343236508977f;  // sin(pi/8)
     constexpr float H = 0.70710678118654752f;   // sqrt(1/2)
-    const C sid = SIGN > 0 ? mul_i(d) : make_float2(d.y, -d.x);  // SIGN * i * d
-    switch (j) {
-        case 0: return d;
-        case 1: return crot(d, C1, s * S1);
-        case 2: return __fmul2_rn(__fadd2_rn(d, sid), make_float2(H, H));
-        case 3: return crot(d, S1, s * C1);
-        case 4: return sid;
-        case 5: return crot(d, -S1, s * C1);
-        case 6: return __fmul2_rn(__fadd2_rn(sid, make_float2(-d.x, -d.y)), make_float2(H, H));
-        default: return crot(d, -C1, s * S1);
-    }
+    if (kb == 0) return make_float2(1.f, 0.f);
+    if (M2 == 8) return make_float2(H, s * H);
+    return kb == 1 ? make_float2(C1, s * S1) : kb == 2 ? make_float2(H, s * H) : make_float2(S1, s * C1);
 }
 
-__host__ __device__ constexpr int bitrev(int r, int R)
+// u = a + T b, v = a - T b with T = (c + i s) (SIGN i)^rot
+template <int SIGN>
+__device__ __forceinline__ void bfly_tw(C& a, C& b, C T, bool rot)
 {
-    int o = 0;
-    for (int b = 1; b < R; b <<= 1) { o = (o << 1) | (r & 1); r >>= 1; }
-    return o;
+    const C sib = SIGN > 0 ? mul_i(b) : make_float2(b.y, -b.x);  // SIGN * i * b
+    C u;
+    if (!rot) {  // T b = c b + s (i b)
+        u = __ffma2_rn(b, make_float2(T.x, T.x), a);
+        u = __ffma2_rn(sib, make_float2((float)SIGN * T.y, (float)SIGN * T.y), u);
+    } else {  // (SIGN i) T b = c (SIGN i b) - SIGN s b
+        u = __ffma2_rn(sib, make_float2(T.x, T.x), a);
+        u = __ffma2_rn(b, make_float2(-(float)SIGN * T.y, -(float)SIGN * T.y), u);
+    }
+    b = __ffma2_rn(a, make_float2(2.f, 2.f), make_float2(-u.x, -u.y));
+    a = u;
 }
 
-// In-register radix-R DFT (decimation in frequency) on slots q + r*S; X[r] ends up in slot q + bitrev(r)*S.
-template <int R, int SIGN>
-__device__ __forceinline__ void butterfly(C (&x)[16], int q)
+// In-register radix-R DFT of slots q + r*S (natural order in, natural order out), input twiddles folded when TW.
+template <int R, int SIGN, bool TW>
+__device__ __forceinline__ void dft_dit(C (&x)[16], int q, const C (&tw)[R / 2])
 {
     constexpr int S = 16 / R;
+    C cur[R];
 #pragma unroll
-    for (int half = R / 2; half >= 1; half >>= 1) {
+    for (int r = 0; r < R; ++r) cur[r] = x[q + r * S];
 #pragma unroll
-        for (int g = 0; g < R; g += 2 * half) {
+    for (int M2 = 2; M2 <= R; M2 <<= 1) {
+        const int s2 = R / M2, M = M2 / 2, quarter = M2 >= 4 ? M2 / 4 : 1;
+        C nxt[R];
 #pragma unroll
-            for (int k = 0; k < half; ++k) {
-                const C u = x[q + (g + k) * S], w = x[q + (g + k + half) * S];
-                x[q + (g + k) * S] = cadd(u, w);
-                x[q + (g + k + half) * S] = mul_w16<SIGN>(csub(u, w), k * (8 / half));
+        for (int o = 0; o < s2; ++o) {
+#pragma unroll
+            for (int k = 0; k < M; ++k) {
+                C a = cur[o + 2 * s2 * k], b = cur[o + s2 + 2 * s2 * k];
+                const int kb = k % quarter;
+                const bool rot = k >= quarter;
+                if (TW) {
+                    bfly_tw<SIGN>(a, b, tw[tw_index(M2, kb)], rot);
+                } else if (kb == 0) {  // T = 1 or SIGN i
+                    const C tb = !rot ? b : (SIGN > 0 ? mul_i(b) : make_float2(b.y, -b.x));
+                    const C u = cadd(a, tb);
+                    b = csub(a, tb);
+                    a = u;
+                } else {
+                    bfly_tw<SIGN>(a, b, w_const<SIGN>(M2, kb), rot);
+                }
+                nxt[o + s2 * k] = a;
+                nxt[o + s2 * (k + M)] = b;
             }
         }
-    }
-}
-
-template <int R, int SIGN>
-__device__ __forceinline__ void pass_butterflies(C (&x)[16])
-{
 #pragma unroll
-    for (int q = 0; q < 16 / R; ++q) butterfly<R, SIGN>(x, q);
+        for (int r = 0; r < R; ++r) cur[r] = nxt[r];
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) x[q + r * S] = cur[r];
 }
 
-// Twiddles of one pass in two steps, so that the serial part (table load, squarings) runs in the window between the
-// scatter and the gather of the preceding exchange, where the thread would otherwise wait at the barrier.
-// prepare = w1 (for radix 16 also the powers 2, 3, 4, 8, 12); apply = the remaining products and x[q + r*S] *= w1^r.
-// Every power is a product of depth <= log2 R.
-template <int R> struct TwSet { C w1[16 / R]; };
-template <> struct TwSet<16> { C w1, w2, w3, w4, w8, w12; };
-
+// The twiddle set of one pass from w = exp(SIGN 2 pi i (j mod NS) / (NS R)): powers by squaring, the rest by products
+// with constants (FMUL2 + FFMA2 with immediates).  Runs in the window between the scatter and the gather of the
+// preceding exchange, where the thread would otherwise wait at the barrier.
 template <int N, int R, int NS, int SIGN>
 __device__ __forceinline__ TwSet<R> twiddle_prepare(int t, const float2* __restrict__ tw)
 {
     constexpr int S = 16 / R;
     constexpr int TPU = N / 16;
     TwSet<R> s;
-    if constexpr (R == 16) {
-        s.w1 = __ldg(&tw[(t & (NS - 1)) * (N / (NS * R))]);
-        if (SIGN > 0) s.w1.y = -s.w1.y;
-        s.w2 = cmul(s.w1, s.w1);
-        s.w3 = cmul(s.w2, s.w1);
-        s.w4 = cmul(s.w2, s.w2);
-        s.w8 = cmul(s.w4, s.w4);
-        s.w12 = cmul(s.w8, s.w4);
-    } else {
 #pragma unroll
-        for (int q = 0; q < S; ++q) {
-            s.w1[q] = __ldg(&tw[((t + q * TPU) & (NS - 1)) * (N / (NS * R))]);
-            if (SIGN > 0) s.w1[q].y = -s.w1[q].y;
+    for (int q = 0; q < S; ++q) {
+        C w = __ldg(&tw[((t + q * TPU) & (NS - 1)) * (N / (NS * R))]);
+        if (SIGN > 0) w.y = -w.y;
+        // w^{R/M2} for M2 = R, R/2, ..., 2
+#pragma unroll
+        for (int M2 = R; M2 >= 2; M2 >>= 1) {
+            s.t[q][tw_index(M2, 0)] = w;
+#pragma unroll
+            for (int kb = 1; kb < M2 / 4; ++kb) {
+                const C k = w_const<SIGN>(M2, kb);
+                s.t[q][tw_index(M2, kb)] = (M2 == 8 || kb == 2)
+                    ? __fmul2_rn(__fadd2_rn(w, SIGN > 0 ? mul_i(w) : make_float2(w.y, -w.x)), make_float2(k.x, k.x))
+                    : crot(w, k.x, k.y);
+            }
+            if (M2 > 2) w = cmul(w, w);
         }
     }
     return s;
 }
 
-template <int R>
-__device__ __forceinline__ void twiddle_apply(C (&x)[16], const TwSet<R>& tw)
+template <int R, int SIGN, bool TW>
+__device__ __forceinline__ void pass_dit(C (&x)[16], const TwSet<TW ? R : 1>& tw)
 {
-    constexpr int S = 16 / R;
-    if constexpr (R == 16) {
-        x[1] = cmul(x[1], tw.w1);
-        x[2] = cmul(x[2], tw.w2);
-        x[3] = cmul(x[3], tw.w3);
-        x[4] = cmul(x[4], tw.w4);
-        x[5] = cmul(x[5], cmul(tw.w4, tw.w1));
-        x[6] = cmul(x[6], cmul(tw.w4, tw.w2));
-        x[7] = cmul(x[7], cmul(tw.w4, tw.w3));
-        x[8] = cmul(x[8], tw.w8);
-        x[9] = cmul(x[9], cmul(tw.w8, tw.w1));
-        x[10] = cmul(x[10], cmul(tw.w8, tw.w2));
-        x[11] = cmul(x[11], cmul(tw.w8, tw.w3));
-        x[12] = cmul(x[12], tw.w12);
-        x[13] = cmul(x[13], cmul(tw.w12, tw.w1));
-        x[14] = cmul(x[14], cmul(tw.w12, tw.w2));
-        x[15] = cmul(x[15], cmul(tw.w12, tw.w3));
-    } else {
 #pragma unroll
-        for (int q = 0; q < S; ++q) {
-#define XR(r) x[q + (r) * S]
-            const C w1 = tw.w1[q];
-            XR(1) = cmul(XR(1), w1);
-            if constexpr (R >= 4) {
-                const C w2 = cmul(w1, w1);
-                const C w3 = cmul(w2, w1);
-                XR(2) = cmul(XR(2), w2);
-                XR(3) = cmul(XR(3), w3);
-                if constexpr (R >= 8) {
-                    const C w4 = cmul(w2, w2);
-                    XR(4) = cmul(XR(4), w4);
-                    XR(5) = cmul(XR(5), cmul(w4, w1));
-                    XR(6) = cmul(XR(6), cmul(w4, w2));
-                    XR(7) = cmul(XR(7), cmul(w4, w3));
-                }
-            }
-#undef XR
+    for (int q = 0; q < 16 / R; ++q) {
+        if constexpr (TW) {
+            dft_dit<R, SIGN, true>(x, q, tw.t[q]);
+        } else {
+            const C none[R / 2] = {};
+            dft_dit<R, SIGN, false>(x, q, none);
         }
     }
 }
@@ -180,7 +184,7 @@ __device__ __forceinline__ void exchange_scatter(const C (&x)[16], int t, C* __r
         const int k = jv & (NS - 1);
         C* base = sm + pad16((jv - k) * R + k);
 #pragma unroll
-        for (int r = 0; r < R; ++r) base[r * STEP] = x[q + bitrev(r, R) * S];
+        for (int r = 0; r < R; ++r) base[r * STEP] = x[q + r * S];
     }
 }
 
@@ -199,20 +203,6 @@ __device__ __forceinline__ void group_bar(int id, int count)
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
 }
 
-// Puts the outputs of a final radix-R pass (left bit-reversed by butterfly()) back into the canonical slot map.
-template <int R>
-__device__ __forceinline__ void natural_order(C (&x)[16])
-{
-    constexpr int S = 16 / R;
-    C y[16];
-#pragma unroll
-    for (int q = 0; q < S; ++q)
-#pragma unroll
-        for (int r = 0; r < R; ++r) y[q + r * S] = x[q + bitrev(r, R) * S];
-#pragma unroll
-    for (int m = 0; m < 16; ++m) x[m] = y[m];
-}
-
 // Full N-point transform (N = R0*R1*R2*R3, R3 = 1 for three passes); unnormalised; kernel exp(SIGN*2*pi*i*k*n/N).
 // tw[m] = exp(-2*pi*i*m/N).  `after_first` runs once between the first barrier and the first gather (the fused kernel
 // issues its input prefetch there).
@@ -221,33 +211,27 @@ __device__ __forceinline__ void fft_aos(C (&x)[16], int t, C* __restrict__ sm, c
                                         int bar_count, F after_first)
 {
     static_assert(R0 * R1 * R2 * R3 == N, "radix plan");
-    pass_butterflies<R0, SIGN>(x);
+    pass_dit<R0, SIGN, false>(x, TwSet<1>{});
     exchange_scatter<N, R0, 1>(x, t, sm);
     const TwSet<R1> tw1 = twiddle_prepare<N, R1, R0, SIGN>(t, tw);
     group_bar(bar_id, bar_count);
     after_first();
     exchange_gather<N>(x, t, sm);
     group_bar(bar_id, bar_count);
-    twiddle_apply<R1>(x, tw1);
-    pass_butterflies<R1, SIGN>(x);
+    pass_dit<R1, SIGN, true>(x, tw1);
     exchange_scatter<N, R1, R0>(x, t, sm);
     const TwSet<R2> tw2 = twiddle_prepare<N, R2, R0 * R1, SIGN>(t, tw);
     group_bar(bar_id, bar_count);
     exchange_gather<N>(x, t, sm);
     group_bar(bar_id, bar_count);
-    twiddle_apply<R2>(x, tw2);
-    pass_butterflies<R2, SIGN>(x);
+    pass_dit<R2, SIGN, true>(x, tw2);
     if constexpr (R3 > 1) {
         exchange_scatter<N, R2, R0 * R1>(x, t, sm);
         const TwSet<R3> tw3 = twiddle_prepare<N, R3, R0 * R1 * R2, SIGN>(t, tw);
         group_bar(bar_id, bar_count);
         exchange_gather<N>(x, t, sm);
         group_bar(bar_id, bar_count);
-        twiddle_apply<R3>(x, tw3);
-        pass_butterflies<R3, SIGN>(x);
-        natural_order<R3>(x);
-    } else {
-        natural_order<R2>(x);
+        pass_dit<R3, SIGN, true>(x, tw3);
     }
 }
 
