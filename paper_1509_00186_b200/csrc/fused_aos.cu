@@ -18,6 +18,9 @@
 // the exchange buffer is reused for the detected powers only after the last gather's barrier, and for the next
 // transform's scatter only after the epilogue's closing barrier; the chirp row is rewritten between two
 // __syncthreads() that all groups reach in the same loop iteration.
+#include <stdio.h>
+#include <stdlib.h>
+
 #include "dedisp_internal.h"
 #include "fft_aos.cuh"
 
@@ -25,17 +28,22 @@ using namespace dedisp_aos;
 
 namespace {
 
-constexpr int CTA = 1024;  // threads per CTA: 64 registers each
-
-// N = R0*R1*R2*R3 (16 elements per thread, N/16 threads per unit); GROUP = threads that share a named barrier and hold
-// U units; CHIRP_SMEM: the channel's chirp row (8 B x N) fits in shared memory beside the exchange buffers.
-template <int N> struct AShape;
-template <> struct AShape<1024>  { static constexpr int GROUP = 256,  U = 4, R0 = 16, R1 = 16, R2 = 4,  R3 = 1; static constexpr bool CHIRP_SMEM = true; };
-template <> struct AShape<2048>  { static constexpr int GROUP = 256,  U = 2, R0 = 16, R1 = 16, R2 = 8,  R3 = 1; static constexpr bool CHIRP_SMEM = true; };
-template <> struct AShape<4096>  { static constexpr int GROUP = 256,  U = 1, R0 = 16, R1 = 16, R2 = 16, R3 = 1; static constexpr bool CHIRP_SMEM = true; };
-template <> struct AShape<8192>  { static constexpr int GROUP = 512,  U = 1, R0 = 16, R1 = 16, R2 = 16, R3 = 2; static constexpr bool CHIRP_SMEM = false; };
-template <> struct AShape<16384> { static constexpr int GROUP = 1024, U = 1, R0 = 16, R1 = 16, R2 = 16, R3 = 4; static constexpr bool CHIRP_SMEM = false; };
-template <int N> __host__ __device__ constexpr int units_per_super_of() { return CTA / AShape<N>::GROUP * AShape<N>::U; }
+// N = R0*R1*R2*R3, E elements per thread (N/E threads per unit), CTA threads per block, GROUP = threads that share a
+// named barrier (they hold GROUP*E/N units); CHIRP_SMEM: the channel's chirp row (8 B x N) fits in shared memory beside
+// the exchange buffers.
+template <int N, int E> struct AShape;
+template <> struct AShape<1024, 16>  { static constexpr int CTA = 1024, GROUP = 256,  R0 = 16, R1 = 16, R2 = 4,  R3 = 1; };
+template <> struct AShape<2048, 16>  { static constexpr int CTA = 1024, GROUP = 256,  R0 = 16, R1 = 16, R2 = 8,  R3 = 1; };
+template <> struct AShape<4096, 16>  { static constexpr int CTA = 1024, GROUP = 256,  R0 = 16, R1 = 16, R2 = 16, R3 = 1; };
+template <> struct AShape<8192, 16>  { static constexpr int CTA = 1024, GROUP = 512,  R0 = 16, R1 = 16, R2 = 16, R3 = 2; };
+template <> struct AShape<16384, 16> { static constexpr int CTA = 1024, GROUP = 1024, R0 = 16, R1 = 16, R2 = 16, R3 = 4; };
+template <> struct AShape<1024, 64>  { static constexpr int CTA = 256, GROUP = 32,  R0 = 64, R1 = 16, R2 = 1, R3 = 1; };
+template <> struct AShape<2048, 64>  { static constexpr int CTA = 256, GROUP = 32,  R0 = 64, R1 = 32, R2 = 1, R3 = 1; };
+template <> struct AShape<4096, 64>  { static constexpr int CTA = 256, GROUP = 64,  R0 = 64, R1 = 64, R2 = 1, R3 = 1; };
+template <> struct AShape<8192, 64>  { static constexpr int CTA = 256, GROUP = 128, R0 = 64, R1 = 64, R2 = 2, R3 = 1; };
+template <> struct AShape<16384, 64> { static constexpr int CTA = 256, GROUP = 256, R0 = 64, R1 = 64, R2 = 4, R3 = 1; };
+template <int N, int E> __host__ __device__ constexpr int units_per_super_of() { return AShape<N, E>::CTA / (N / E); }
+template <int N> __host__ __device__ constexpr bool chirp_in_smem() { return N <= 4096; }
 
 struct AosArgs {
     const int8_t* xt;      // [n_chan][xt_stride][2]
@@ -45,12 +53,12 @@ struct AosArgs {
     float* out;            // [n_dm][n_chan][out_stride]
     long long out_stride, out_col0;
     int accumulate;        // add to out instead of overwriting it (second polarisation)
-    float2* spec;          // [gridDim.x][4U][N] forward-spectrum stash, used when n_dm > 1
+    float2* spec;          // [gridDim.x][units per super-item][N] forward-spectrum stash, used when n_dm > 1
     float2* volt;          // debug: [n_dm][L] voltages of block volt_block, else nullptr
     int volt_block;
     int dump_unpack;       // debug (with volt != nullptr): store the registers right after unpack_int8x2 as [N] (re, im)
     int nb;                // blocks per channel
-    int spc;               // super-items per channel = ceil(nb / 4U)
+    int spc;               // super-items per channel = ceil(nb / units per super-item)
     int n_super;           // super-items to process
     int first_super;       // debug: start here
     int n_chan, n_dm, log2_nint, head, L;
@@ -75,34 +83,35 @@ __device__ __forceinline__ C unpack_int8x2(uint32_t v)
     return __fadd2_rn(make_float2(__uint_as_float(re), __uint_as_float(im)), make_float2(-8388736.0f, -8388736.0f));
 }
 
-template <int N> constexpr size_t smem_bytes()
+template <int N, int E> constexpr size_t smem_bytes()
 {
-    return (size_t)units_per_super_of<N>() * (sizeof(float2) * padded_len(N) + N * sizeof(uint16_t)) +
-           (AShape<N>::CHIRP_SMEM ? sizeof(float2) * N : 0);
+    return (size_t)units_per_super_of<N, E>() * (sizeof(float2) * padp<AShape<N, E>::R0>(N) + N * sizeof(uint16_t)) +
+           (chirp_in_smem<N>() ? sizeof(float2) * N : 0);
 }
 
 // LGN = log2(n_int) when it is one of the specialised values (the epilogue then has no run-time geometry), else -1.
-template <int N, int LGN>
-__global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
+template <int N, int E, int LGN>
+__global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const AosArgs a)
 {
-    using Sh = AShape<N>;
-    constexpr int GROUP = Sh::GROUP, TPU = N / 16, UPS = units_per_super_of<N>();
-    constexpr bool CHIRP_SMEM = Sh::CHIRP_SMEM;
+    using Sh = AShape<N, E>;
+    constexpr int CTA = Sh::CTA, GROUP = Sh::GROUP, TPU = N / E, UPS = units_per_super_of<N, E>(), P = Sh::R0;
+    constexpr bool CHIRP_SMEM = chirp_in_smem<N>();
     extern __shared__ float2 smem2[];
-    const int g = threadIdx.x / GROUP;  // group: its own barrier
-    const int us = threadIdx.x / TPU;   // unit slot inside the super-item (g*U + unit in group)
+    const int us = threadIdx.x / TPU;   // unit slot inside the super-item
     const int t = threadIdx.x % TPU;    // thread inside the unit
-    const int bar_id = g + 1;
-    C* sm = smem2 + (size_t)us * padded_len(N);                         // exchange buffer of this unit
+    const int bar_id = threadIdx.x / GROUP + 1;  // the group's own named barrier
+    C* sm = smem2 + (size_t)us * padp<P>(N);                             // exchange buffer of this unit
     float* smf = reinterpret_cast<float*>(sm);                           // ... reused for the detected powers
-    float2* chirp_s = smem2 + (size_t)UPS * padded_len(N);               // [N], whole CTA (only if CHIRP_SMEM)
+    float2* chirp_s = smem2 + (size_t)UPS * padp<P>(N);                  // [N], whole CTA (only if CHIRP_SMEM)
     uint16_t* stage = reinterpret_cast<uint16_t*>(chirp_s + (CHIRP_SMEM ? N : 0)) + (size_t)us * N;  // [N] int8 pairs
     const uint16_t* xt16 = reinterpret_cast<const uint16_t*>(a.xt);
 
     const int lgn = LGN >= 0 ? LGN : a.log2_nint;
     const int n_out = a.L >> lgn;
-    // epilogue geometry: each lane sums 2^lg_chunk consecutive samples, 2^lg_lpo lanes make one output
-    const int lg_chunk = lgn < 2 ? lgn : (lgn > 7 ? lgn - 5 : 2);
+    // epilogue geometry: each lane sums 2^lg_chunk consecutive samples, 2^lg_lpo lanes (inside one unit's threads and
+    // one warp) make one output
+    constexpr int MAX_LPO = TPU >= 32 ? 5 : 4;
+    const int lg_chunk = lgn < 2 ? lgn : (lgn > 2 + MAX_LPO ? lgn - MAX_LPO : 2);
     const int lg_lpo = lgn - lg_chunk;
     const int n_work = a.L >> lg_chunk;
 
@@ -114,7 +123,7 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
     const int s_begin = a.first_super + (CHIRP_SMEM ? (int)((long long)blockIdx.x * a.n_super / gridDim.x) : (int)blockIdx.x);
     const int s_end = a.first_super + (CHIRP_SMEM ? (int)((long long)(blockIdx.x + 1) * a.n_super / gridDim.x) : a.n_super);
 
-    // stage the int8 rows of this thread's unit of super-item s: 2 x 16 B per thread (P:L270 framing: block b reads
+    // stage the int8 rows of this thread's unit of super-item s: E/8 x 16 B per thread (P:L270 framing: block b reads
     // rows b*L .. b*L+N-1; consecutive blocks overlap)
     auto prefetch = [&](int s) {
         const int c = s / a.spc;
@@ -122,7 +131,7 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
         if (b < a.nb) {
             const uint16_t* src = xt16 + (long long)c * a.xt_stride + (long long)b * a.L;
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
+            for (int j = 0; j < E / 8; ++j) {
                 const int k = (j * TPU + t) * 8;  // 8 samples = 16 B
                 cp_async16(stage + k, src + k);
             }
@@ -151,50 +160,49 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
         }
         // (the staged rows of this super-item are complete and visible: see the barrier that ends the previous one)
 
+        C x[E];
+        float2* stash = a.spec + ((size_t)blockIdx.x * UPS + us) * N;
         // 1b. unpack int8 (re, im) -> fp32 (exact)
-        C x[16];
 #pragma unroll
-        for (int m = 0; m < 16; ++m) x[m] = unpack_int8x2(live ? (uint32_t)stage[t + m * TPU] : 0u);
-        if (a.volt && a.dump_unpack) {  // debug hook (one super-item): what the transform is about to see, bit for bit
+        for (int m = 0; m < E; ++m) x[m] = unpack_int8x2(live ? (uint32_t)stage[t + m * TPU] : 0u);
+        if (a.volt && a.dump_unpack) {  // debug hook (one super-item): what the transform is about to see
             if (live && a.volt_block == b) {
 #pragma unroll
-                for (int m = 0; m < 16; ++m) a.volt[t + m * TPU] = x[m];
+                for (int m = 0; m < E; ++m) a.volt[t + m * TPU] = x[m];
             }
-            return;  // uniform over the CTA; no cp.async is in flight (the prefetch is issued inside the transform)
+            return;  // uniform over the CTA; no cp.async is in flight (the prefetch is issued in the transform)
         }
-
         // 2. forward FFT; once every thread of the group is past the unpack, the staging buffer is
         //    free for the next super-item's rows
-        fft_aos<N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, -1>(x, t, sm, a.tw, bar_id, GROUP, [&] {
+        fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, -1>(x, t, sm, a.tw, bar_id, GROUP, [&] {
             if (s + s_step < s_end) prefetch(s + s_step);
         });
-
-        float2* stash = a.spec + ((size_t)blockIdx.x * UPS + us) * N;
         if (a.n_dm > 1) {
 #pragma unroll
-            for (int m = 0; m < 16; ++m) stash[t + m * TPU] = x[m];
+            for (int m = 0; m < E; ++m) stash[t + m * TPU] = x[m];
         }
+#pragma unroll 1
         for (int d = 0; d < a.n_dm; ++d) {
             if (d > 0) {
 #pragma unroll
-                for (int m = 0; m < 16; ++m) x[m] = stash[t + m * TPU];  // same thread wrote it: no fence needed
+                for (int m = 0; m < E; ++m) x[m] = stash[t + m * TPU];  // same thread wrote it: no fence needed
             }
             // 3. chirp multiply (Eq. 3)
             if (CHIRP_SMEM && a.n_dm == 1) {
 #pragma unroll
-                for (int m = 0; m < 16; ++m) x[m] = cmul(x[m], chirp_s[t + m * TPU]);
+                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], chirp_s[t + m * TPU]);
             } else {
-                const float2* h = a.chirp + ((size_t)d * a.n_chan + c) * N + t;
+                const float2* hp = a.chirp + ((size_t)d * a.n_chan + c) * N + t;
 #pragma unroll
-                for (int m = 0; m < 16; ++m) x[m] = cmul(x[m], __ldg(h + m * TPU));
+                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], __ldg(hp + m * TPU));
             }
-            // 4. inverse FFT (1/N already applied)
-            fft_aos<N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, +1>(x, t, sm, a.tw, bar_id, GROUP, [] {});
+            // 4. inverse FFT (1/N already in the chirp)
+            fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, +1>(x, t, sm, a.tw, bar_id, GROUP, [] {});
 
             if (a.volt) {  // debug hook: valid voltages of one block
                 if (live && a.volt_block == b) {
 #pragma unroll
-                    for (int m = 0; m < 16; ++m) {
+                    for (int m = 0; m < E; ++m) {
                         const int i = t + m * TPU - a.head;
                         if (i >= 0 && i < a.L) a.volt[(size_t)d * a.L + i] = x[m];
                     }
@@ -205,7 +213,7 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
             }
             // 5 + 6. discard the overlap, detect, integrate n_int samples (R9, R11)
 #pragma unroll
-            for (int m = 0; m < 16; ++m) {
+            for (int m = 0; m < E; ++m) {
                 const float2 sq = __fmul2_rn(x[m], x[m]);
                 smf[t + m * TPU] = sq.x + sq.y;
             }
@@ -239,7 +247,7 @@ __global__ void __launch_bounds__(CTA, 1) fused_aos_kernel(const AosArgs a)
     }
 }
 
-struct KernelInfo { int ctas_per_sm; int n_sm; size_t spec_bytes; };
+struct KernelInfo { int e; int ctas_per_sm; int n_sm; size_t spec_bytes; };
 KernelInfo g_info[5];
 bool g_init_done = false;
 
@@ -251,68 +259,78 @@ int slot_of(int n_fft)
     }
 }
 
-template <int N, int LGN> int set_smem()
+template <int N, int E, int LGN> int set_smem()
 {
-    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_aos_kernel<N, LGN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem_bytes<N>()));
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_aos_kernel<N, E, LGN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem_bytes<N, E>()));
     return DEDISP_OK;
 }
 
-template <int N> int init_one(int slot)
+template <int N, int E> int init_one(int slot)
 {
     int rc;
-    if ((rc = set_smem<N, -1>()) || (rc = set_smem<N, 2>()) || (rc = set_smem<N, 3>()) || (rc = set_smem<N, 4>()) ||
-        (rc = set_smem<N, 5>()) || (rc = set_smem<N, 6>()))
+    if ((rc = set_smem<N, E, -1>()) || (rc = set_smem<N, E, 2>()) || (rc = set_smem<N, E, 3>()) ||
+        (rc = set_smem<N, E, 4>()) || (rc = set_smem<N, E, 5>()) || (rc = set_smem<N, E, 6>()))
         return rc;
     int occ = 0;
-    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_aos_kernel<N, -1>, CTA, smem_bytes<N>()));
+    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_aos_kernel<N, E, -1>, AShape<N, E>::CTA,
+                                                                  smem_bytes<N, E>()));
     int dev = 0, n_sm = 0;
     DEDISP_CUDA_TRY(cudaGetDevice(&dev));
     DEDISP_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    g_info[slot].e = E;
     g_info[slot].ctas_per_sm = occ > 0 ? occ : 1;
     g_info[slot].n_sm = n_sm;
-    g_info[slot].spec_bytes = sizeof(float2) * (size_t)g_info[slot].ctas_per_sm * n_sm * units_per_super_of<N>() * N;
+    g_info[slot].spec_bytes = sizeof(float2) * (size_t)g_info[slot].ctas_per_sm * n_sm * units_per_super_of<N, E>() * N;
     return DEDISP_OK;
 }
 
-template <int N>
+template <int N, int E>
 int launch_one(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
 {
     const int slot = slot_of(N);
     long long grid = (long long)g_info[slot].ctas_per_sm * g_info[slot].n_sm;
     if (grid > a.n_super) grid = a.n_super;
     a.spec = p->d_spec;
-    const dim3 g((unsigned)grid), b(CTA);
+    const dim3 g((unsigned)grid), b(AShape<N, E>::CTA);
+    constexpr size_t sb = smem_bytes<N, E>();
     switch (a.volt ? -1 : a.log2_nint) {  // n_int = 4 ... 64 (the five BASELINE configs) are specialised
-        case 2: fused_aos_kernel<N, 2><<<g, b, smem_bytes<N>(), st>>>(a); break;
-        case 3: fused_aos_kernel<N, 3><<<g, b, smem_bytes<N>(), st>>>(a); break;
-        case 4: fused_aos_kernel<N, 4><<<g, b, smem_bytes<N>(), st>>>(a); break;
-        case 5: fused_aos_kernel<N, 5><<<g, b, smem_bytes<N>(), st>>>(a); break;
-        case 6: fused_aos_kernel<N, 6><<<g, b, smem_bytes<N>(), st>>>(a); break;
-        default: fused_aos_kernel<N, -1><<<g, b, smem_bytes<N>(), st>>>(a); break;
+        case 2: fused_aos_kernel<N, E, 2><<<g, b, sb, st>>>(a); break;
+        case 3: fused_aos_kernel<N, E, 3><<<g, b, sb, st>>>(a); break;
+        case 4: fused_aos_kernel<N, E, 4><<<g, b, sb, st>>>(a); break;
+        case 5: fused_aos_kernel<N, E, 5><<<g, b, sb, st>>>(a); break;
+        case 6: fused_aos_kernel<N, E, 6><<<g, b, sb, st>>>(a); break;
+        default: fused_aos_kernel<N, E, -1><<<g, b, sb, st>>>(a); break;
     }
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;
 }
 
+template <int N> int launch_n(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
+{
+    return g_info[slot_of(N)].e == 64 ? launch_one<N, 64>(p, a, st) : launch_one<N, 16>(p, a, st);
+}
+
 int dispatch(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
 {
     switch (p->n_fft) {
-        case 1024: return launch_one<1024>(p, a, st);
-        case 2048: return launch_one<2048>(p, a, st);
-        case 4096: return launch_one<4096>(p, a, st);
-        case 8192: return launch_one<8192>(p, a, st);
-        case 16384: return launch_one<16384>(p, a, st);
+        case 1024: return launch_n<1024>(p, a, st);
+        case 2048: return launch_n<2048>(p, a, st);
+        case 4096: return launch_n<4096>(p, a, st);
+        case 8192: return launch_n<8192>(p, a, st);
+        case 16384: return launch_n<16384>(p, a, st);
         default: return DEDISP_EINVAL;
     }
 }
 
+template <int N> int ups_n(int e) { return e == 64 ? units_per_super_of<N, 64>() : units_per_super_of<N, 16>(); }
 int units_per_super(int n_fft)
 {
+    const int e = g_info[slot_of(n_fft)].e;
     switch (n_fft) {
-        case 1024: return units_per_super_of<1024>(); case 2048: return units_per_super_of<2048>();
-        case 4096: return units_per_super_of<4096>(); case 8192: return units_per_super_of<8192>();
-        default: return units_per_super_of<16384>();
+        case 1024: return ups_n<1024>(e); case 2048: return ups_n<2048>(e);
+        case 4096: return ups_n<4096>(e); case 8192: return ups_n<8192>(e);
+        default: return ups_n<16384>(e);
     }
 }
 
@@ -340,12 +358,17 @@ size_t dedisp_aos_spec_bytes(int n_fft)
     return slot < 0 ? 0 : g_info[slot].spec_bytes;
 }
 
+template <int N> int init_n(int slot, int e) { return e == 64 ? init_one<N, 64>(slot) : init_one<N, 16>(slot); }
+
 int dedisp_aos_init(void)
 {
     if (g_init_done) return DEDISP_OK;
+    // elements per thread for N = 1024 ... 16384 (EXPERIMENT: override with DEDISP_AOS_E="e0,e1,e2,e3,e4")
+    int e[5] = {64, 64, 64, 16, 16};
+    if (const char* env = getenv("DEDISP_AOS_E")) sscanf(env, "%d,%d,%d,%d,%d", &e[0], &e[1], &e[2], &e[3], &e[4]);
     int rc;
-    if ((rc = init_one<1024>(0)) || (rc = init_one<2048>(1)) || (rc = init_one<4096>(2)) || (rc = init_one<8192>(3)) ||
-        (rc = init_one<16384>(4)))
+    if ((rc = init_n<1024>(0, e[0])) || (rc = init_n<2048>(1, e[1])) || (rc = init_n<4096>(2, e[2])) ||
+        (rc = init_n<8192>(3, e[3])) || (rc = init_n<16384>(4, e[4])))
         return rc;
     g_init_done = true;
     return DEDISP_OK;
