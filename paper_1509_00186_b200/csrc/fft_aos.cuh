@@ -75,6 +75,19 @@ __device__ __forceinline__ C w_const(int kb)
     return make_float2(cos64(j), (float)SIGN * cos64(16 - j));
 }
 
+// 2a - u in one FFMA2.  Written in PTX on 64-bit registers: with the intrinsic, ptxas copies about a quarter of these
+// results to a scratch register pair before they are stored to shared memory (MOV, MOV, STS.64 on one pair, serialised).
+__device__ __forceinline__ C two_a_minus(C a, C u)
+{
+    unsigned long long ra, ru, rv;
+    C v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ru) : "f"(-u.x), "f"(-u.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rv) : "l"(ra), "l"(0x4000000040000000ull), "l"(ru));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(v.x), "=f"(v.y) : "l"(rv));
+    return v;
+}
+
 // u = a + T b, v = a - T b with T = (c + i s) (SIGN i)^rot
 template <int SIGN>
 __device__ __forceinline__ void bfly_tw(C& a, C& b, C T, bool rot)
@@ -88,7 +101,7 @@ __device__ __forceinline__ void bfly_tw(C& a, C& b, C T, bool rot)
         u = __ffma2_rn(sib, make_float2(T.x, T.x), a);
         u = __ffma2_rn(b, make_float2(-(float)SIGN * T.y, -(float)SIGN * T.y), u);
     }
-    b = __ffma2_rn(a, make_float2(2.f, 2.f), make_float2(-u.x, -u.y));
+    b = two_a_minus(a, u);
     a = u;
 }
 

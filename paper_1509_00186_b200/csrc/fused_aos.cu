@@ -90,12 +90,20 @@ template <int N, int E> constexpr size_t smem_bytes()
 }
 
 // LGN = log2(n_int) when it is one of the specialised values (the epilogue then has no run-time geometry), else -1.
-template <int N, int E, int LGN>
+// MODE: the three control flows are separate instantiations, so that the hot loop of each is straight-line code with
+// the spectrum in fixed registers (a merged loop costs ~100 register moves per unit at the join points).
+enum { MODE_ONE_DM = 0, MODE_MULTI_DM = 1, MODE_DEBUG = 2 };
+template <int N, int E, int LGN, int MODE>
+#ifdef QLB
+__global__ void __launch_bounds__(QLB, 1) fused_aos_kernel(const AosArgs a)
+#else
 __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const AosArgs a)
+#endif
 {
     using Sh = AShape<N, E>;
     constexpr int CTA = Sh::CTA, GROUP = Sh::GROUP, TPU = N / E, UPS = units_per_super_of<N, E>(), P = Sh::R0;
     constexpr bool CHIRP_SMEM = chirp_in_smem<N>();
+    constexpr bool ROW_SMEM = CHIRP_SMEM && MODE == MODE_ONE_DM;  // the channel's chirp row is held in shared memory
     extern __shared__ float2 smem2[];
     const int us = threadIdx.x / TPU;   // unit slot inside the super-item
     const int t = threadIdx.x % TPU;    // thread inside the unit
@@ -151,7 +159,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
         const int b = (s - c * a.spc) * UPS + us;
         const bool live = b < a.nb;
 
-        if (CHIRP_SMEM && a.n_dm == 1 && c != cur_chan) {  // all groups take this branch in the same iteration
+        if (ROW_SMEM && c != cur_chan) {  // all groups take this branch in the same iteration
             __syncthreads();
             const float2* row = a.chirp + (size_t)c * N;
             for (int i = threadIdx.x; i < N; i += CTA) chirp_s[i] = __ldg(row + i);
@@ -161,11 +169,10 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
         // (the staged rows of this super-item are complete and visible: see the barrier that ends the previous one)
 
         C x[E];
-        float2* stash = a.spec + ((size_t)blockIdx.x * UPS + us) * N;
         // 1b. unpack int8 (re, im) -> fp32 (exact)
 #pragma unroll
         for (int m = 0; m < E; ++m) x[m] = unpack_int8x2(live ? (uint32_t)stage[t + m * TPU] : 0u);
-        if (a.volt && a.dump_unpack) {  // debug hook (one super-item): what the transform is about to see
+        if (MODE == MODE_DEBUG && a.dump_unpack) {  // debug hook (one super-item): what the transform is about to see
             if (live && a.volt_block == b) {
 #pragma unroll
                 for (int m = 0; m < E; ++m) a.volt[t + m * TPU] = x[m];
@@ -177,18 +184,11 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
         fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, -1>(x, t, sm, a.tw, bar_id, GROUP, [&] {
             if (s + s_step < s_end) prefetch(s + s_step);
         });
-        if (a.n_dm > 1) {
-#pragma unroll
-            for (int m = 0; m < E; ++m) stash[t + m * TPU] = x[m];
-        }
-#pragma unroll 1
-        for (int d = 0; d < a.n_dm; ++d) {
-            if (d > 0) {
-#pragma unroll
-                for (int m = 0; m < E; ++m) x[m] = stash[t + m * TPU];  // same thread wrote it: no fence needed
-            }
+
+        // steps 3-6 for trial DM d on the spectrum in x
+        auto dedisperse = [&](int d) {
             // 3. chirp multiply (Eq. 3)
-            if (CHIRP_SMEM && a.n_dm == 1) {
+            if (ROW_SMEM) {
 #pragma unroll
                 for (int m = 0; m < E; ++m) x[m] = cmul(x[m], chirp_s[t + m * TPU]);
             } else {
@@ -199,7 +199,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
             // 4. inverse FFT (1/N already in the chirp)
             fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, +1>(x, t, sm, a.tw, bar_id, GROUP, [] {});
 
-            if (a.volt) {  // debug hook: valid voltages of one block
+            if constexpr (MODE == MODE_DEBUG) {  // debug hook: valid voltages of one block
                 if (live && a.volt_block == b) {
 #pragma unroll
                     for (int m = 0; m < E; ++m) {
@@ -209,8 +209,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
                 }
                 cp_async_wait_all();
                 group_bar(bar_id, GROUP);
-                continue;
-            }
+            } else {
             // 5 + 6. discard the overlap, detect, integrate n_int samples (R9, R11)
 #pragma unroll
             for (int m = 0; m < E; ++m) {
@@ -219,34 +218,88 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
             }
             group_bar(bar_id, GROUP);
             float* dst = a.out + ((size_t)d * a.n_chan + c) * a.out_stride + a.out_col0 + (long long)b * n_out;
-            for (int id = t; id - t < n_work; id += TPU) {  // uniform trip count: the shuffles need whole warps
-                float acc = 0.f;
-                if (id < n_work) {
-                    const float* p0 = smf + a.head + (id << lg_chunk);  // head % min(n_int, 4) == 0: aligned
-                    if (lg_chunk >= 2) {
-                        for (int j = 0; j < (1 << lg_chunk); j += 4) {
-                            const float4 u = *reinterpret_cast<const float4*>(p0 + j);
-                            acc += (u.x + u.y) + (u.z + u.w);
-                        }
-                    } else if (lg_chunk == 1) {
-                        const float2 u = *reinterpret_cast<const float2*>(p0);
-                        acc = u.x + u.y;
-                    } else {
-                        acc = p0[0];
+            if constexpr (LGN >= 2) {
+                // chunk id = t + i*TPU holds 4 consecutive powers (one LDS.128); 2^LPO lanes make one output, which
+                // lands at (t >> LPO) + i*(TPU >> LPO): base + compile-time stride, no index arithmetic in the loop
+                constexpr int LPO = LGN - 2;
+                static_assert(LPO <= MAX_LPO, "the lanes of one output sit in one warp and one unit");
+                const float4* p4 = reinterpret_cast<const float4*>(smf + a.head) + t;  // head % 4 == 0
+                float* dt = dst + (t >> LPO);
+                const bool writer = live && (t & ((1 << LPO) - 1)) == 0;
+                const int n_full = n_work / TPU, rem = n_work - n_full * TPU;
+                auto one = [&](int i, bool valid) {
+                    float acc = 0.f;
+                    if (valid) {
+                        const float4 u = p4[i * TPU];
+                        acc = (u.x + u.y) + (u.z + u.w);
                     }
+#pragma unroll
+                    for (int off = 1; off < (1 << LPO); off <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+                    if (writer && valid) {
+                        float* q = dt + i * (TPU >> LPO);
+                        *q = a.accumulate ? *q + acc : acc;
+                    }
+                };
+#pragma unroll 4
+                for (int i = 0; i < n_full; ++i) one(i, true);
+                if (rem > 0) one(n_full, t < rem);  // rem % 2^LPO == 0 (L % n_int == 0): whole lane groups
+            } else {
+                for (int id = t; id - t < n_work; id += TPU) {  // uniform trip count: the shuffles need whole warps
+                    float acc = 0.f;
+                    if (id < n_work) {
+                        const float* p0 = smf + a.head + (id << lg_chunk);  // head % min(n_int, 4) == 0: aligned
+                        if (lg_chunk >= 2) {
+                            for (int j = 0; j < (1 << lg_chunk); j += 4) {
+                                const float4 u = *reinterpret_cast<const float4*>(p0 + j);
+                                acc += (u.x + u.y) + (u.z + u.w);
+                            }
+                        } else if (lg_chunk == 1) {
+                            const float2 u = *reinterpret_cast<const float2*>(p0);
+                            acc = u.x + u.y;
+                        } else {
+                            acc = p0[0];
+                        }
+                    }
+                    for (int off = 1; off < (1 << lg_lpo); off <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+                    if (live && id < n_work && (id & ((1 << lg_lpo) - 1)) == 0)
+                        dst[id >> lg_lpo] = a.accumulate ? dst[id >> lg_lpo] + acc : acc;
                 }
-                for (int off = 1; off < (1 << lg_lpo); off <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-                if (live && id < n_work && (id & ((1 << lg_lpo) - 1)) == 0)
-                    dst[id >> lg_lpo] = a.accumulate ? dst[id >> lg_lpo] + acc : acc;
             }
             // one barrier for two hand-overs: the powers live in the exchange buffer of the next transform, and the
             // rows prefetched for the next super-item (issued during this one's first exchange) become visible
             cp_async_wait_all();
             group_bar(bar_id, GROUP);
+            }
+        };
+
+        if constexpr (MODE == MODE_ONE_DM) {
+            dedisperse(0);
+        } else {
+            // the forward spectrum is computed once and shared by all trial DMs: every DM reads it back from the
+            // (L2-resident) stash; the same thread wrote it, so no fence is needed
+            // (the debug instantiation also serves single-DM plans, which have no stash)
+            const bool use_stash = MODE == MODE_MULTI_DM || a.n_dm > 1;
+            float2* stash = a.spec + ((size_t)blockIdx.x * UPS + us) * N;
+            if (use_stash) {
+#pragma unroll
+                for (int m = 0; m < E; ++m) stash[t + m * TPU] = x[m];
+            }
+#pragma unroll 1
+            for (int d = 0; d < a.n_dm; ++d) {
+                if (use_stash) {
+#pragma unroll
+                    for (int m = 0; m < E; ++m) x[m] = stash[t + m * TPU];
+                }
+                dedisperse(d);
+            }
         }
     }
 }
 
+#ifdef DEDISP_QUICK  // local experiments: one instantiation only (nvcc -DDEDISP_QUICK -DQN=4096 -DQE=64 -DQL=2)
+template __global__ void fused_aos_kernel<QN, QE, QL, QM>(const AosArgs);
+}
+#else
 struct KernelInfo { int e; int ctas_per_sm; int n_sm; size_t spec_bytes; };
 KernelInfo g_info[5];
 bool g_init_done = false;
@@ -259,22 +312,38 @@ int slot_of(int n_fft)
     }
 }
 
-template <int N, int E, int LGN> int set_smem()
+// The specialised epilogue is built for the n_int of the BASELINE.json workload of each transform size only (tiny,
+// gmrt16, gmrt32, lowfreq / wideband); every other n_int runs the generic epilogue (LGN = -1).
+template <int N> constexpr int special_lgn(int which) { return -1; }
+template <> constexpr int special_lgn<1024>(int) { return 4; }
+template <> constexpr int special_lgn<2048>(int) { return 3; }
+template <> constexpr int special_lgn<4096>(int) { return 2; }
+template <> constexpr int special_lgn<16384>(int which) { return which == 0 ? 5 : 6; }
+
+template <int N, int E, int LGN, int MODE> int set_smem()
 {
-    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_aos_kernel<N, E, LGN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_aos_kernel<N, E, LGN, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem_bytes<N, E>()));
+    return DEDISP_OK;
+}
+template <int N, int E, int LGN> int set_smem_modes()
+{
+    int rc;
+    if ((rc = set_smem<N, E, LGN, MODE_ONE_DM>()) || (rc = set_smem<N, E, LGN, MODE_MULTI_DM>())) return rc;
     return DEDISP_OK;
 }
 
 template <int N, int E> int init_one(int slot)
 {
     int rc;
-    if ((rc = set_smem<N, E, -1>()) || (rc = set_smem<N, E, 2>()) || (rc = set_smem<N, E, 3>()) ||
-        (rc = set_smem<N, E, 4>()) || (rc = set_smem<N, E, 5>()) || (rc = set_smem<N, E, 6>()))
-        return rc;
+    if ((rc = set_smem_modes<N, E, -1>()) || (rc = set_smem<N, E, -1, MODE_DEBUG>())) return rc;
+    if constexpr (special_lgn<N>(0) >= 0)
+        if ((rc = set_smem_modes<N, E, special_lgn<N>(0)>())) return rc;
+    if constexpr (special_lgn<N>(1) != special_lgn<N>(0))
+        if ((rc = set_smem_modes<N, E, special_lgn<N>(1)>())) return rc;
     int occ = 0;
-    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_aos_kernel<N, E, -1>, AShape<N, E>::CTA,
-                                                                  smem_bytes<N, E>()));
+    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_aos_kernel<N, E, -1, MODE_MULTI_DM>,
+                                                                  AShape<N, E>::CTA, smem_bytes<N, E>()));
     int dev = 0, n_sm = 0;
     DEDISP_CUDA_TRY(cudaGetDevice(&dev));
     DEDISP_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
@@ -285,6 +354,15 @@ template <int N, int E> int init_one(int slot)
     return DEDISP_OK;
 }
 
+template <int N, int E, int LGN>
+void launch_lgn(const AosArgs& a, int n_dm, dim3 g, cudaStream_t st)
+{
+    const dim3 b(AShape<N, E>::CTA);
+    constexpr size_t sb = smem_bytes<N, E>();
+    if (n_dm == 1) fused_aos_kernel<N, E, LGN, MODE_ONE_DM><<<g, b, sb, st>>>(a);
+    else fused_aos_kernel<N, E, LGN, MODE_MULTI_DM><<<g, b, sb, st>>>(a);
+}
+
 template <int N, int E>
 int launch_one(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
 {
@@ -292,15 +370,15 @@ int launch_one(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
     long long grid = (long long)g_info[slot].ctas_per_sm * g_info[slot].n_sm;
     if (grid > a.n_super) grid = a.n_super;
     a.spec = p->d_spec;
-    const dim3 g((unsigned)grid), b(AShape<N, E>::CTA);
-    constexpr size_t sb = smem_bytes<N, E>();
-    switch (a.volt ? -1 : a.log2_nint) {  // n_int = 4 ... 64 (the five BASELINE configs) are specialised
-        case 2: fused_aos_kernel<N, E, 2><<<g, b, sb, st>>>(a); break;
-        case 3: fused_aos_kernel<N, E, 3><<<g, b, sb, st>>>(a); break;
-        case 4: fused_aos_kernel<N, E, 4><<<g, b, sb, st>>>(a); break;
-        case 5: fused_aos_kernel<N, E, 5><<<g, b, sb, st>>>(a); break;
-        case 6: fused_aos_kernel<N, E, 6><<<g, b, sb, st>>>(a); break;
-        default: fused_aos_kernel<N, E, -1><<<g, b, sb, st>>>(a); break;
+    const dim3 g((unsigned)grid);
+    if (a.volt) {
+        fused_aos_kernel<N, E, -1, MODE_DEBUG><<<g, dim3(AShape<N, E>::CTA), smem_bytes<N, E>(), st>>>(a);
+    } else if (special_lgn<N>(0) >= 0 && a.log2_nint == special_lgn<N>(0)) {
+        launch_lgn<N, E, special_lgn<N>(0)>(a, p->n_dm, g, st);
+    } else if (special_lgn<N>(1) >= 0 && a.log2_nint == special_lgn<N>(1)) {
+        launch_lgn<N, E, special_lgn<N>(1)>(a, p->n_dm, g, st);
+    } else {
+        launch_lgn<N, E, -1>(a, p->n_dm, g, st);
     }
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;
@@ -398,3 +476,4 @@ int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, 
     a.dump_unpack = dump_unpack;
     return dispatch(p, a, st);
 }
+#endif  // DEDISP_QUICK
