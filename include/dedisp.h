@@ -20,7 +20,11 @@
  *
  * Pointers: every pointer argument says HOST or DEVICE.  The library never takes ownership of caller buffers.
  * Errors:   every call returns DEDISP_OK (0) or a negative DEDISP_E* code; no exceptions, no aborts, no output.
- * Threads:  a plan may be used from one host thread at a time.
+ * Threads:  a plan may be used from one host thread at a time, and its calls must be ordered on ONE stream at a time
+ *           (a plan owns scratch buffers that its kernels share; two executes of one plan on two streams would race).
+ *           Plans are independent of each other.
+ * Devices:  a plan belongs to the device that was current in dedisp_plan(); every later call on it must be made with
+ *           that device current (else DEDISP_EINVAL).  Several devices may be used from one process.
  */
 #ifndef DEDISP_H
 #define DEDISP_H

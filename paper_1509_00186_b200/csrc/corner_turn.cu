@@ -1,7 +1,9 @@
 // corner_turn.cu -- step 1a of the path: the GSB voltage-beam block arrives time-major, int8 [t][chan][re,im]
 // (R10).  Every later step works on one channel's time series, so the block is turned once into
 // channel-major int8 [chan][t][re,im] (2 B per complex sample stay 2 B: the unpack to fp32 happens in registers of the
-// fused kernel).  Pure byte movement: bit-exact by construction.  HBM-bound: 2 B read + 2 B written per sample.
+// fused kernel).  Byte movement plus one bit flip: every byte is stored as x ^ 0x80 (= x + 128 as an unsigned byte), the
+// form the fused kernel's I2F-free conversion starts from; the flip is free in this HBM-bound kernel and saves the
+// fused kernel one LOP3 per sample.  HBM-bound: 2 B read + 2 B written per sample.
 #include "dedisp_internal.h"
 
 namespace {
@@ -32,6 +34,7 @@ __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const int8_t* __re
         uint4 v = make_uint4(0, 0, 0, 0);
         if (t >= 0 && t < n_samp && c < n_chan)  // n_chan % 8 == 0: the 8 channels are all inside
             v = __ldg(reinterpret_cast<const uint4*>(in16 + t * n_chan + c));
+        v.x ^= 0x80808080u; v.y ^= 0x80808080u; v.z ^= 0x80808080u; v.w ^= 0x80808080u;
         uint32_t* dst = &tile[row * PITCH_W + q * 4];
         dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
     }
@@ -78,7 +81,7 @@ __global__ void __launch_bounds__(256) corner_turn_scalar_kernel(const int8_t* _
     for (int r = y; r < 32; r += 8) {
         const long long t = t0 + r;
         const int c = c0 + x;
-        tile[r][x] = (t < n_samp && c < n_chan) ? in16[t * n_chan + c] : (uint16_t)0;
+        tile[r][x] = (t < n_samp && c < n_chan) ? (uint16_t)(in16[t * n_chan + c] ^ 0x8080u) : (uint16_t)0x8080u;
     }
     __syncthreads();
     for (int r = y; r < 32; r += 8) {

@@ -234,12 +234,14 @@ __device__ __forceinline__ void group_bar(int id, int count)
 // Full N-point transform (N = R0*R1*R2*R3, trailing radices 1 when unused); unnormalised; kernel
 // exp(SIGN*2*pi*i*k*n/N).  `after_first` runs once between the first barrier and the first gather (the fused kernel
 // issues its input prefetch there).  Every gather is followed by a barrier, so on return the exchange buffer is free.
-template <int E, int N, int R0, int R1, int R2, int R3, int SIGN, class F>
+// PRE_BAR: the buffer is still being read by the caller on entry; a barrier is placed before the first scatter.
+template <int E, int N, int R0, int R1, int R2, int R3, int SIGN, bool PRE_BAR, class F>
 __device__ __forceinline__ void fft_aos(C (&x)[E], int t, C* __restrict__ sm, const float2* __restrict__ tw, int bar_id,
                                         int bar_count, F after_first)
 {
     static_assert(R0 * R1 * R2 * R3 == N, "radix plan");
     pass_dit<E, R0, SIGN, false>(x, TwBase<E, R0>{});
+    if (PRE_BAR) group_bar(bar_id, bar_count);  // the caller's last reads of the exchange buffer end here
     exchange_scatter<E, N, R0, 1, R0>(x, t, sm);
     const TwBase<E, R1> tw1 = twiddle_load<E, N, R1, R0, SIGN>(t, tw);
     group_bar(bar_id, bar_count);
@@ -248,19 +250,19 @@ __device__ __forceinline__ void fft_aos(C (&x)[E], int t, C* __restrict__ sm, co
     group_bar(bar_id, bar_count);
     pass_dit<E, R1, SIGN, true>(x, tw1);
     if constexpr (R2 > 1) {
-        exchange_scatter<E, N, R1, R0, R0>(x, t, sm);
+            exchange_scatter<E, N, R1, R0, R0>(x, t, sm);
         const TwBase<E, R2> tw2 = twiddle_load<E, N, R2, R0 * R1, SIGN>(t, tw);
         group_bar(bar_id, bar_count);
         exchange_gather<E, N, R0>(x, t, sm);
         group_bar(bar_id, bar_count);
-        pass_dit<E, R2, SIGN, true>(x, tw2);
+            pass_dit<E, R2, SIGN, true>(x, tw2);
         if constexpr (R3 > 1) {
-            exchange_scatter<E, N, R2, R0 * R1, R0>(x, t, sm);
+                    exchange_scatter<E, N, R2, R0 * R1, R0>(x, t, sm);
             const TwBase<E, R3> tw3 = twiddle_load<E, N, R3, R0 * R1 * R2, SIGN>(t, tw);
             group_bar(bar_id, bar_count);
             exchange_gather<E, N, R0>(x, t, sm);
             group_bar(bar_id, bar_count);
-            pass_dit<E, R3, SIGN, true>(x, tw3);
+                    pass_dit<E, R3, SIGN, true>(x, tw3);
         }
     }
 }

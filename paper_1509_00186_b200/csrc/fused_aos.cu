@@ -4,22 +4,28 @@
 // registers and shared memory.  Every complex number is one packed f32x2 register pair (fft_aos.cuh), so the arithmetic
 // is FADD2/FMUL2/FFMA2.  The forward spectrum is computed once per (channel, block) and shared by all trial DMs.
 //
-// 16 elements per thread = 32 data registers (64 in all), N/16 threads per (channel, block) unit, ONE persistent
-// 1024-thread CTA per SM split into groups that own their units, exchange buffers and a named barrier: four groups of
-// 256 threads for N <= 4096 (1/2/4 units each), two of 512 for N = 8192, one of 1024 for N = 16384.  While one group is
-// in a shared-memory exchange the others keep the FP32 pipe busy.  A CTA walks a contiguous range of "super-items"
-// (consecutive blocks of ONE channel, one per unit slot):
+// 64 elements per thread (128 data registers, ~190-215 in all), N/64 threads per (channel, block) unit, ONE persistent
+// 256-thread CTA per SM holding 256*64/N units at a time (4 at N = 4096), each with its own exchange buffer and barrier
+// (a named barrier over the unit's threads; a warp barrier when the unit fits in one warp, N <= 2048).  A 4096-point
+// transform is two radix-64 passes with ONE trip through shared memory; with 16 elements per thread and 1024 threads
+// (the round-1 shape) it was three passes and two trips, and the shared-memory data pipe was the first limiter
+// (profiles/r2_*).  A CTA walks a contiguous range of "super-items" (consecutive blocks of ONE channel, one per unit):
 //   * for N <= 4096 the channel's chirp row sits in shared memory and is reloaded only when the channel changes
 //     (larger rows do not fit beside the exchange buffers and come from L2);
-//   * the int8 rows of the NEXT super-item are prefetched with cp.async while this one computes.
-// Barrier discipline (compute-sanitizer is not available on this pool, so it is spelled out): a group's staging rows
-// are written by cp.async issued after the first barrier of the forward transform (every thread of the group is then
-// past its unpack reads) and become visible at the barrier that ends the super-item (cp.async.wait_group 0 before it);
-// the exchange buffer is reused for the detected powers only after the last gather's barrier, and for the next
-// transform's scatter only after the epilogue's closing barrier; the chirp row is rewritten between two
-// __syncthreads() that all groups reach in the same loop iteration.
-#include <stdio.h>
-#include <stdlib.h>
+//   * the int8 rows of the NEXT super-item are prefetched with cp.async while this one computes;
+//   * single-DM plans unpack the next super-item beside the epilogue of this one (PIPE below): with two warps per SM
+//     sub-partition nothing else hides the shared-memory latency of the epilogue.
+// The three control flows (one DM, several DMs, debug hooks) are separate instantiations (MODE), so the hot loop of each
+// is straight-line code with the spectrum in fixed registers.
+// Barrier discipline (compute-sanitizer is not available on this pool, so it is spelled out): a unit's staging rows
+// are written by cp.async issued after the first barrier of the forward transform (every thread of the unit is then
+// past its unpack reads: those sit before that transform in program order) and become visible at the barrier between
+// the power stores and the power reads of the epilogue (PIPE; cp.async.wait_group 0 before it) or at the barrier that
+// ends the super-item (otherwise); the exchange buffer is reused for the detected powers only after the last gather's
+// barrier, and for the next transform's scatter only after the epilogue's closing barrier (PIPE: the barrier the
+// forward transform places before its first scatter); the chirp row is rewritten between two __syncthreads() that all
+// units reach in the same loop iteration.
+#include <mutex>
 
 #include "dedisp_internal.h"
 #include "fft_aos.cuh"
@@ -29,20 +35,22 @@ using namespace dedisp_aos;
 namespace {
 
 // N = R0*R1*R2*R3, E elements per thread (N/E threads per unit), CTA threads per block, GROUP = threads that share a
-// named barrier (they hold GROUP*E/N units); CHIRP_SMEM: the channel's chirp row (8 B x N) fits in shared memory beside
-// the exchange buffers.
+// barrier (a named barrier, or a warp barrier when a unit fits in a warp).
+// STAGE: the int8 rows of the next super-item are prefetched into shared memory with cp.async (else read from global
+// memory when the unit starts); ROW: single-DM plans keep the channel's chirp row in shared memory (else it comes from
+// L2: 8 B x N does not fit beside the exchange buffers for N > 4096).
 template <int N, int E> struct AShape;
-template <> struct AShape<1024, 16>  { static constexpr int CTA = 1024, GROUP = 256,  R0 = 16, R1 = 16, R2 = 4,  R3 = 1; };
-template <> struct AShape<2048, 16>  { static constexpr int CTA = 1024, GROUP = 256,  R0 = 16, R1 = 16, R2 = 8,  R3 = 1; };
-template <> struct AShape<4096, 16>  { static constexpr int CTA = 1024, GROUP = 256,  R0 = 16, R1 = 16, R2 = 16, R3 = 1; };
-template <> struct AShape<8192, 16>  { static constexpr int CTA = 1024, GROUP = 512,  R0 = 16, R1 = 16, R2 = 16, R3 = 2; };
-template <> struct AShape<16384, 16> { static constexpr int CTA = 1024, GROUP = 1024, R0 = 16, R1 = 16, R2 = 16, R3 = 4; };
 template <> struct AShape<1024, 64>  { static constexpr int CTA = 256, GROUP = 32,  R0 = 64, R1 = 16, R2 = 1, R3 = 1; };
 template <> struct AShape<2048, 64>  { static constexpr int CTA = 256, GROUP = 32,  R0 = 64, R1 = 32, R2 = 1, R3 = 1; };
 template <> struct AShape<4096, 64>  { static constexpr int CTA = 256, GROUP = 64,  R0 = 64, R1 = 64, R2 = 1, R3 = 1; };
 template <> struct AShape<8192, 64>  { static constexpr int CTA = 256, GROUP = 128, R0 = 64, R1 = 64, R2 = 2, R3 = 1; };
 template <> struct AShape<16384, 64> { static constexpr int CTA = 256, GROUP = 256, R0 = 64, R1 = 64, R2 = 4, R3 = 1; };
-template <int N, int E> __host__ __device__ constexpr int units_per_super_of() { return AShape<N, E>::CTA / (N / E); }
+template <int N, int E> struct Cfg {
+    static constexpr int CTA = AShape<N, E>::CTA;
+    static constexpr bool STAGE = true, ROW = N <= 4096;
+};
+constexpr int AOS_E = 64;  // elements per thread of every built size (E = 16 was measured slower on all five workloads)
+template <int N, int E> __host__ __device__ constexpr int units_per_super_of() { return Cfg<N, E>::CTA / (N / E); }
 template <int N> __host__ __device__ constexpr bool chirp_in_smem() { return N <= 4096; }
 
 struct AosArgs {
@@ -72,11 +80,11 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// int8 pair (re | im << 8) -> fp32 (re, im), exact, without I2F: bytes ^ 0x80 -> 0x4B0000uu = 2^23 + u (u = x + 128),
-// then one packed add of -(2^23 + 128)
-__device__ __forceinline__ C unpack_int8x2(uint32_t v)
+// biased int8 pair ((re ^ 0x80) | (im ^ 0x80) << 8, as the corner turn stores it: u = x + 128) -> fp32 (re, im), exact,
+// without I2F: PRMT builds 0x4B0000uu = 2^23 + u, then one packed add of -(2^23 + 128)
+__device__ __forceinline__ C unpack_int8x2(uint32_t w)
 {
-    const uint32_t w = v ^ 0x8080u, k = 0x4B000000u;
+    const uint32_t k = 0x4B000000u;
     uint32_t re, im;
     asm("prmt.b32 %0, %1, %2, 0x7440;" : "=r"(re) : "r"(w), "r"(k));
     asm("prmt.b32 %0, %1, %2, 0x7441;" : "=r"(im) : "r"(w), "r"(k));
@@ -85,8 +93,9 @@ __device__ __forceinline__ C unpack_int8x2(uint32_t v)
 
 template <int N, int E> constexpr size_t smem_bytes()
 {
-    return (size_t)units_per_super_of<N, E>() * (sizeof(float2) * padp<AShape<N, E>::R0>(N) + N * sizeof(uint16_t)) +
-           (chirp_in_smem<N>() ? sizeof(float2) * N : 0);
+    return (size_t)units_per_super_of<N, E>() *
+               (sizeof(float2) * padp<AShape<N, E>::R0>(N) + (Cfg<N, E>::STAGE ? N * sizeof(uint16_t) : 0)) +
+           (Cfg<N, E>::ROW ? sizeof(float2) * N : 0);
 }
 
 // LGN = log2(n_int) when it is one of the specialised values (the epilogue then has no run-time geometry), else -1.
@@ -94,16 +103,13 @@ template <int N, int E> constexpr size_t smem_bytes()
 // the spectrum in fixed registers (a merged loop costs ~100 register moves per unit at the join points).
 enum { MODE_ONE_DM = 0, MODE_MULTI_DM = 1, MODE_DEBUG = 2 };
 template <int N, int E, int LGN, int MODE>
-#ifdef QLB
-__global__ void __launch_bounds__(QLB, 1) fused_aos_kernel(const AosArgs a)
-#else
-__global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const AosArgs a)
-#endif
+__global__ void __launch_bounds__((Cfg<N, E>::CTA), 1) fused_aos_kernel(const AosArgs a)
 {
     using Sh = AShape<N, E>;
-    constexpr int CTA = Sh::CTA, GROUP = Sh::GROUP, TPU = N / E, UPS = units_per_super_of<N, E>(), P = Sh::R0;
-    constexpr bool CHIRP_SMEM = chirp_in_smem<N>();
-    constexpr bool ROW_SMEM = CHIRP_SMEM && MODE == MODE_ONE_DM;  // the channel's chirp row is held in shared memory
+    constexpr int CTA = Cfg<N, E>::CTA, GROUP = Sh::GROUP, TPU = N / E, UPS = units_per_super_of<N, E>(), P = Sh::R0;
+    constexpr bool CHIRP_SMEM = chirp_in_smem<N>();  // decides the work split (see below)
+    constexpr bool STAGE = Cfg<N, E>::STAGE;
+    constexpr bool ROW_SMEM = Cfg<N, E>::ROW && MODE == MODE_ONE_DM;  // the channel's chirp row is held in shared memory
     extern __shared__ float2 smem2[];
     const int us = threadIdx.x / TPU;   // unit slot inside the super-item
     const int t = threadIdx.x % TPU;    // thread inside the unit
@@ -111,7 +117,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
     C* sm = smem2 + (size_t)us * padp<P>(N);                             // exchange buffer of this unit
     float* smf = reinterpret_cast<float*>(sm);                           // ... reused for the detected powers
     float2* chirp_s = smem2 + (size_t)UPS * padp<P>(N);                  // [N], whole CTA (only if CHIRP_SMEM)
-    uint16_t* stage = reinterpret_cast<uint16_t*>(chirp_s + (CHIRP_SMEM ? N : 0)) + (size_t)us * N;  // [N] int8 pairs
+    uint16_t* stage = reinterpret_cast<uint16_t*>(chirp_s + (Cfg<N, E>::ROW ? N : 0)) + (size_t)us * N;  // [N] int8 pairs
     const uint16_t* xt16 = reinterpret_cast<const uint16_t*>(a.xt);
 
     const int lgn = LGN >= 0 ? LGN : a.log2_nint;
@@ -134,6 +140,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
     // stage the int8 rows of this thread's unit of super-item s: E/8 x 16 B per thread (P:L270 framing: block b reads
     // rows b*L .. b*L+N-1; consecutive blocks overlap)
     auto prefetch = [&](int s) {
+        if (!STAGE) return;
         const int c = s / a.spc;
         const int b = (s - c * a.spc) * UPS + us;
         if (b < a.nb) {
@@ -148,11 +155,31 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
     };
 
     int cur_chan = -1;
-    if (s_begin < s_end) {
+    if (STAGE && s_begin < s_end) {
         prefetch(s_begin);
         cp_async_wait_all();
         group_bar(bar_id, GROUP);
     }
+
+    // 1b. unpack int8 (re, im) -> fp32 (exact) for this thread's unit of super-item s2
+    C x[E];
+    auto unpack = [&](int s2) {
+        const int c2 = s2 / a.spc;
+        const int b2 = (s2 - c2 * a.spc) * UPS + us;
+        const bool live2 = b2 < a.nb;
+        if constexpr (STAGE) {
+#pragma unroll
+            for (int m = 0; m < E; ++m) x[m] = unpack_int8x2(live2 ? (uint32_t)stage[t + m * TPU] : 0u);
+        } else {  // block b reads rows b*L .. b*L+N-1 (P:L270 framing)
+            const uint16_t* src = xt16 + (long long)c2 * a.xt_stride + (long long)b2 * a.L + t;
+#pragma unroll
+            for (int m = 0; m < E; ++m) x[m] = unpack_int8x2(live2 ? (uint32_t)__ldg(src + m * TPU) : 0u);
+        }
+    };
+    // PIPE (single-DM plans): the unpack of the NEXT super-item runs beside the epilogue of this one, whose
+    // shared-memory round trip (powers out, barrier, sums in) would otherwise leave the warp idle
+    constexpr bool PIPE = MODE == MODE_ONE_DM && STAGE;
+    if (PIPE && s_begin < s_end) unpack(s_begin);
 
     for (int s = s_begin; s < s_end; s += s_step) {
         const int c = s / a.spc;
@@ -168,10 +195,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
         }
         // (the staged rows of this super-item are complete and visible: see the barrier that ends the previous one)
 
-        C x[E];
-        // 1b. unpack int8 (re, im) -> fp32 (exact)
-#pragma unroll
-        for (int m = 0; m < E; ++m) x[m] = unpack_int8x2(live ? (uint32_t)stage[t + m * TPU] : 0u);
+        if (!PIPE) unpack(s);
         if (MODE == MODE_DEBUG && a.dump_unpack) {  // debug hook (one super-item): what the transform is about to see
             if (live && a.volt_block == b) {
 #pragma unroll
@@ -181,7 +205,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
         }
         // 2. forward FFT; once every thread of the group is past the unpack, the staging buffer is
         //    free for the next super-item's rows
-        fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, -1>(x, t, sm, a.tw, bar_id, GROUP, [&] {
+        fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, -1, PIPE>(x, t, sm, a.tw, bar_id, GROUP, [&] {
             if (s + s_step < s_end) prefetch(s + s_step);
         });
 
@@ -197,7 +221,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
                 for (int m = 0; m < E; ++m) x[m] = cmul(x[m], __ldg(hp + m * TPU));
             }
             // 4. inverse FFT (1/N already in the chirp)
-            fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, +1>(x, t, sm, a.tw, bar_id, GROUP, [] {});
+            fft_aos<E, N, Sh::R0, Sh::R1, Sh::R2, Sh::R3, +1, false>(x, t, sm, a.tw, bar_id, GROUP, [] {});
 
             if constexpr (MODE == MODE_DEBUG) {  // debug hook: valid voltages of one block
                 if (live && a.volt_block == b) {
@@ -216,6 +240,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
                 const float2 sq = __fmul2_rn(x[m], x[m]);
                 smf[t + m * TPU] = sq.x + sq.y;
             }
+            if (PIPE) cp_async_wait_all();  // the next super-item's rows become visible at this barrier too
             group_bar(bar_id, GROUP);
             float* dst = a.out + ((size_t)d * a.n_chan + c) * a.out_stride + a.out_col0 + (long long)b * n_out;
             if constexpr (LGN >= 2) {
@@ -226,6 +251,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
                 const float4* p4 = reinterpret_cast<const float4*>(smf + a.head) + t;  // head % 4 == 0
                 float* dt = dst + (t >> LPO);
                 const bool writer = live && (t & ((1 << LPO) - 1)) == 0;
+                if (PIPE && s + s_step < s_end) unpack(s + s_step);  // beside the shared-memory reads below
                 const int n_full = n_work / TPU, rem = n_work - n_full * TPU;
                 auto one = [&](int i, bool valid) {
                     float acc = 0.f;
@@ -242,7 +268,7 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
                 };
 #pragma unroll 4
                 for (int i = 0; i < n_full; ++i) one(i, true);
-                if (rem > 0) one(n_full, t < rem);  // rem % 2^LPO == 0 (L % n_int == 0): whole lane groups
+                if (rem > 0) one(n_full, t < rem);
             } else {
                 for (int id = t; id - t < n_work; id += TPU) {  // uniform trip count: the shuffles need whole warps
                     float acc = 0.f;
@@ -264,11 +290,14 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
                     if (live && id < n_work && (id & ((1 << lg_lpo) - 1)) == 0)
                         dst[id >> lg_lpo] = a.accumulate ? dst[id >> lg_lpo] + acc : acc;
                 }
+                if (PIPE && s + s_step < s_end) unpack(s + s_step);
             }
             // one barrier for two hand-overs: the powers live in the exchange buffer of the next transform, and the
             // rows prefetched for the next super-item (issued during this one's first exchange) become visible
-            cp_async_wait_all();
-            group_bar(bar_id, GROUP);
+            if (!PIPE) {  // (PIPE: the forward transform places this barrier before its first scatter)
+                cp_async_wait_all();
+                group_bar(bar_id, GROUP);
+            }
             }
         };
 
@@ -296,13 +325,13 @@ __global__ void __launch_bounds__((AShape<N, E>::CTA), 1) fused_aos_kernel(const
     }
 }
 
-#ifdef DEDISP_QUICK  // local experiments: one instantiation only (nvcc -DDEDISP_QUICK -DQN=4096 -DQE=64 -DQL=2)
-template __global__ void fused_aos_kernel<QN, QE, QL, QM>(const AosArgs);
-}
-#else
-struct KernelInfo { int e; int ctas_per_sm; int n_sm; size_t spec_bytes; };
-KernelInfo g_info[5];
-bool g_init_done = false;
+// Per-device launch geometry.  The dynamic shared memory attribute of a kernel is a per-device setting and the SM count a
+// per-device fact, so both are established once per device (under a mutex: plans may be made from several host threads).
+struct KernelInfo { int ctas_per_sm; int n_sm; size_t spec_bytes; };
+constexpr int MAX_DEVICES = 64;
+struct DeviceInfo { bool done; KernelInfo k[5]; };
+DeviceInfo g_dev[MAX_DEVICES];
+std::mutex g_dev_mutex;
 
 int slot_of(int n_fft)
 {
@@ -320,95 +349,89 @@ template <> constexpr int special_lgn<2048>(int) { return 3; }
 template <> constexpr int special_lgn<4096>(int) { return 2; }
 template <> constexpr int special_lgn<16384>(int which) { return which == 0 ? 5 : 6; }
 
-template <int N, int E, int LGN, int MODE> int set_smem()
+template <int N, int LGN, int MODE> int set_smem()
 {
-    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_aos_kernel<N, E, LGN, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem_bytes<N, E>()));
+    DEDISP_CUDA_TRY(cudaFuncSetAttribute(fused_aos_kernel<N, AOS_E, LGN, MODE>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<N, AOS_E>()));
     return DEDISP_OK;
 }
-template <int N, int E, int LGN> int set_smem_modes()
+template <int N, int LGN> int set_smem_modes()
 {
     int rc;
-    if ((rc = set_smem<N, E, LGN, MODE_ONE_DM>()) || (rc = set_smem<N, E, LGN, MODE_MULTI_DM>())) return rc;
+    if ((rc = set_smem<N, LGN, MODE_ONE_DM>()) || (rc = set_smem<N, LGN, MODE_MULTI_DM>())) return rc;
     return DEDISP_OK;
 }
 
-template <int N, int E> int init_one(int slot)
+template <int N> int init_one(KernelInfo& k, int dev)
 {
     int rc;
-    if ((rc = set_smem_modes<N, E, -1>()) || (rc = set_smem<N, E, -1, MODE_DEBUG>())) return rc;
+    if ((rc = set_smem_modes<N, -1>()) || (rc = set_smem<N, -1, MODE_DEBUG>())) return rc;
     if constexpr (special_lgn<N>(0) >= 0)
-        if ((rc = set_smem_modes<N, E, special_lgn<N>(0)>())) return rc;
+        if ((rc = set_smem_modes<N, special_lgn<N>(0)>())) return rc;
     if constexpr (special_lgn<N>(1) != special_lgn<N>(0))
-        if ((rc = set_smem_modes<N, E, special_lgn<N>(1)>())) return rc;
-    int occ = 0;
-    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_aos_kernel<N, E, -1, MODE_MULTI_DM>,
-                                                                  AShape<N, E>::CTA, smem_bytes<N, E>()));
-    int dev = 0, n_sm = 0;
-    DEDISP_CUDA_TRY(cudaGetDevice(&dev));
+        if ((rc = set_smem_modes<N, special_lgn<N>(1)>())) return rc;
+    int occ = 0, n_sm = 0;
+    DEDISP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_aos_kernel<N, AOS_E, -1, MODE_MULTI_DM>,
+                                                                  Cfg<N, AOS_E>::CTA, smem_bytes<N, AOS_E>()));
     DEDISP_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    g_info[slot].e = E;
-    g_info[slot].ctas_per_sm = occ > 0 ? occ : 1;
-    g_info[slot].n_sm = n_sm;
-    g_info[slot].spec_bytes = sizeof(float2) * (size_t)g_info[slot].ctas_per_sm * n_sm * units_per_super_of<N, E>() * N;
+    k.ctas_per_sm = occ > 0 ? occ : 1;
+    k.n_sm = n_sm;
+    k.spec_bytes = sizeof(float2) * (size_t)k.ctas_per_sm * n_sm * units_per_super_of<N, AOS_E>() * N;
     return DEDISP_OK;
 }
 
-template <int N, int E, int LGN>
+template <int N, int LGN>
 void launch_lgn(const AosArgs& a, int n_dm, dim3 g, cudaStream_t st)
 {
-    const dim3 b(AShape<N, E>::CTA);
-    constexpr size_t sb = smem_bytes<N, E>();
-    if (n_dm == 1) fused_aos_kernel<N, E, LGN, MODE_ONE_DM><<<g, b, sb, st>>>(a);
-    else fused_aos_kernel<N, E, LGN, MODE_MULTI_DM><<<g, b, sb, st>>>(a);
+    const dim3 b(Cfg<N, AOS_E>::CTA);
+    constexpr size_t sb = smem_bytes<N, AOS_E>();
+    if (n_dm == 1) fused_aos_kernel<N, AOS_E, LGN, MODE_ONE_DM><<<g, b, sb, st>>>(a);
+    else fused_aos_kernel<N, AOS_E, LGN, MODE_MULTI_DM><<<g, b, sb, st>>>(a);
 }
 
-template <int N, int E>
+template <int N>
 int launch_one(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
 {
-    const int slot = slot_of(N);
-    long long grid = (long long)g_info[slot].ctas_per_sm * g_info[slot].n_sm;
+    const KernelInfo& k = g_dev[p->device].k[slot_of(N)];
+    long long grid = (long long)k.ctas_per_sm * k.n_sm;
     if (grid > a.n_super) grid = a.n_super;
     a.spec = p->d_spec;
     const dim3 g((unsigned)grid);
     if (a.volt) {
-        fused_aos_kernel<N, E, -1, MODE_DEBUG><<<g, dim3(AShape<N, E>::CTA), smem_bytes<N, E>(), st>>>(a);
+        fused_aos_kernel<N, AOS_E, -1, MODE_DEBUG><<<g, dim3(Cfg<N, AOS_E>::CTA), smem_bytes<N, AOS_E>(), st>>>(a);
     } else if (special_lgn<N>(0) >= 0 && a.log2_nint == special_lgn<N>(0)) {
-        launch_lgn<N, E, special_lgn<N>(0)>(a, p->n_dm, g, st);
+        launch_lgn<N, special_lgn<N>(0)>(a, p->n_dm, g, st);
     } else if (special_lgn<N>(1) >= 0 && a.log2_nint == special_lgn<N>(1)) {
-        launch_lgn<N, E, special_lgn<N>(1)>(a, p->n_dm, g, st);
+        launch_lgn<N, special_lgn<N>(1)>(a, p->n_dm, g, st);
     } else {
-        launch_lgn<N, E, -1>(a, p->n_dm, g, st);
+        launch_lgn<N, -1>(a, p->n_dm, g, st);
     }
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;
 }
 
-template <int N> int launch_n(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
-{
-    return g_info[slot_of(N)].e == 64 ? launch_one<N, 64>(p, a, st) : launch_one<N, 16>(p, a, st);
-}
-
 int dispatch(const dedisp_plan_s* p, AosArgs& a, cudaStream_t st)
 {
+    // the kernels, their shared-memory attributes and the plan's tables all belong to the plan's device
+    int dev = -1;
+    DEDISP_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != p->device || dev < 0 || dev >= MAX_DEVICES || !g_dev[dev].done) return DEDISP_EINVAL;
     switch (p->n_fft) {
-        case 1024: return launch_n<1024>(p, a, st);
-        case 2048: return launch_n<2048>(p, a, st);
-        case 4096: return launch_n<4096>(p, a, st);
-        case 8192: return launch_n<8192>(p, a, st);
-        case 16384: return launch_n<16384>(p, a, st);
+        case 1024: return launch_one<1024>(p, a, st);
+        case 2048: return launch_one<2048>(p, a, st);
+        case 4096: return launch_one<4096>(p, a, st);
+        case 8192: return launch_one<8192>(p, a, st);
+        case 16384: return launch_one<16384>(p, a, st);
         default: return DEDISP_EINVAL;
     }
 }
 
-template <int N> int ups_n(int e) { return e == 64 ? units_per_super_of<N, 64>() : units_per_super_of<N, 16>(); }
 int units_per_super(int n_fft)
 {
-    const int e = g_info[slot_of(n_fft)].e;
     switch (n_fft) {
-        case 1024: return ups_n<1024>(e); case 2048: return ups_n<2048>(e);
-        case 4096: return ups_n<4096>(e); case 8192: return ups_n<8192>(e);
-        default: return ups_n<16384>(e);
+        case 1024: return units_per_super_of<1024, AOS_E>(); case 2048: return units_per_super_of<2048, AOS_E>();
+        case 4096: return units_per_super_of<4096, AOS_E>(); case 8192: return units_per_super_of<8192, AOS_E>();
+        default: return units_per_super_of<16384, AOS_E>();
     }
 }
 
@@ -432,23 +455,25 @@ int dedisp_aos_supported(int n_fft) { return slot_of(n_fft) >= 0; }
 
 size_t dedisp_aos_spec_bytes(int n_fft)
 {
+    int dev = -1;
     const int slot = slot_of(n_fft);
-    return slot < 0 ? 0 : g_info[slot].spec_bytes;
+    if (slot < 0 || cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES || !g_dev[dev].done) return 0;
+    return g_dev[dev].k[slot].spec_bytes;
 }
-
-template <int N> int init_n(int slot, int e) { return e == 64 ? init_one<N, 64>(slot) : init_one<N, 16>(slot); }
 
 int dedisp_aos_init(void)
 {
-    if (g_init_done) return DEDISP_OK;
-    // elements per thread for N = 1024 ... 16384 (EXPERIMENT: override with DEDISP_AOS_E="e0,e1,e2,e3,e4")
-    int e[5] = {64, 64, 64, 16, 16};
-    if (const char* env = getenv("DEDISP_AOS_E")) sscanf(env, "%d,%d,%d,%d,%d", &e[0], &e[1], &e[2], &e[3], &e[4]);
+    int dev = -1;
+    DEDISP_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return DEDISP_ENODEV;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    DeviceInfo& d = g_dev[dev];
+    if (d.done) return DEDISP_OK;
     int rc;
-    if ((rc = init_n<1024>(0, e[0])) || (rc = init_n<2048>(1, e[1])) || (rc = init_n<4096>(2, e[2])) ||
-        (rc = init_n<8192>(3, e[3])) || (rc = init_n<16384>(4, e[4])))
+    if ((rc = init_one<1024>(d.k[0], dev)) || (rc = init_one<2048>(d.k[1], dev)) || (rc = init_one<4096>(d.k[2], dev)) ||
+        (rc = init_one<8192>(d.k[3], dev)) || (rc = init_one<16384>(d.k[4], dev)))
         return rc;
-    g_init_done = true;
+    d.done = true;
     return DEDISP_OK;
 }
 
@@ -476,4 +501,3 @@ int dedisp_launch_aos_debug_voltage(const dedisp_plan_s* p, const int8_t* d_xt, 
     a.dump_unpack = dump_unpack;
     return dispatch(p, a, st);
 }
-#endif  // DEDISP_QUICK
