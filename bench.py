@@ -71,6 +71,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--workload", default="gmrt32")
+    ap.add_argument("--shard", choices=("batches", "channels"), default="batches",
+                    help="N > 1: one workload-sized batch per rank (weak scaling, default) or one channel range of ONE "
+                         "workload per rank (strong scaling, dedisp_plan_shard; SURVEY 8(e), P:L256-258)")
     ap.add_argument("--duration", type=float, default=0.0, help="override the workload's seconds of data (debug)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -155,7 +158,21 @@ def get_workload(args, rank: int):
     w = datagen.WORKLOADS[args.workload]
     if args.duration > 0:
         w = w.scaled(args.duration)
+    if getattr(args, "shard", "batches") == "channels":
+        return w                                   # strong scaling: every rank a channel range of the SAME batch
     return replace(w, seed=w.seed + rank)          # weak scaling: every rank its own batch
+
+
+def channel_shard(n_chan: int, rank: int, world: int):
+    """(first channel, number of channels) of rank's contiguous channel range; the ranges tile [0, n_chan)."""
+    c0 = rank * n_chan // world
+    return c0, (rank + 1) * n_chan // world - c0
+
+
+def sub_band(w, c0: int, n: int):
+    """The workload restricted to channels c0 .. c0+n-1 (same channel width, shifted centre frequency)."""
+    dv = w.chan_width_hz
+    return replace(w, n_chan=n, bw_hz=n * dv, f_center_hz=w.f_center_hz - 0.5 * w.bw_hz + (c0 + 0.5 * n) * dv)
 
 
 def framing_counts(head: int, tail: int, L: int, n_samp: int, n_fft: int):
@@ -297,13 +314,23 @@ def run_ours(args):
     import datagen
     import paper_1509_00186_b200 as dd          # raises if libdedisp.so is missing: no fallback
 
-    w = get_workload(args, rank)
-    x = datagen.generate(w)                                       # int8 [T][C][2], seeded, host
+    w_band = get_workload(args, rank)
+    by_channels = args.shard == "channels"
+    if by_channels:
+        # rank r holds columns c0 .. c0+n-1 of the band (a host-side slice: here generated directly) and plans them
+        # with the WHOLE band's framing, so all ranks share one time axis; no data-path collective in the step
+        c0, n_loc = channel_shard(w_band.n_chan, rank, world)
+        x = datagen.generate(w_band, chans=range(c0, c0 + n_loc))  # int8 [T][n_loc][2], seeded, host
+        plan = dd.dedisp_plan_shard(w_band.n_chan, w_band.bw_hz, w_band.f_center_hz, w_band.dm_trials, w_band.n_fft,
+                                    w_band.n_int, c0, n_loc)
+        w = sub_band(w_band, c0, n_loc)                           # what this rank processes
+    else:
+        w = w_band
+        x = datagen.generate(w)                                   # int8 [T][C][2], seeded, host
+        plan = dd.dedisp_plan(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
     T = x.shape[0]
     h_in = torch.from_numpy(x).pin_memory()
     d_in = h_in.cuda(non_blocking=False)
-
-    plan = dd.dedisp_plan(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
     head, tail, L = plan.head, plan.tail, plan.L
     nb = plan.n_blocks(T)
     n_out = plan.out_samples(T)
@@ -344,6 +371,10 @@ def run_ours(args):
     clocks = sampler.stop(mark0, max(mark1, mark0 + 1)) if sampler else None
     ms_step = ms_total / args.steps
     value = whole_job_value(samples, world, ms_step * 1e-3)
+    if by_channels and world > 1:  # channel ranges may differ by one channel: sum the ranks' sample counts
+        tot = torch.tensor([float(samples)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tot)
+        value = float(tot.item()) / (ms_step * 1e-3) / 1e6
     checksum = float(d_out[:, :, : min(n_out, 1000)].double().mean().item())   # touches the result; sanity only
 
     # ---- end to end from pinned host memory (config 3: 1 s chunks, double buffered) -------------------------------
@@ -398,7 +429,7 @@ def run_ours(args):
         del d_tmp
         e2e = {"value": world * samples / dt / 1e6, "unit": UNIT,
                "h2d_bytes_per_step": int(h_in.numel()), "d2h_bytes_per_step": int(h_out.numel() * 4),
-               "ms_per_step": dt * 1e3, "real_time_factor": world * samples / dt / w.bw_hz,
+               "ms_per_step": dt * 1e3, "real_time_factor": world * samples / dt / w_band.bw_hz,
                "chunk_samples": chunk, "chunks_per_step": (T + chunk - 1) // chunk,
                "timer": "host wall clock around all pushes + stream_sync",
                "api": "dedisp_stream_push (pinned host int8 in, pinned host fp32 out)",
@@ -447,6 +478,23 @@ def run_ours(args):
                     "algorithmic_bytes_per_launch": b_bytes, "achieved_gbs": b_bytes / (b_ms * 1e-3) / 1e9,
                     "note": "output of the step is 510 MB: partly L2-resident between launches" if d_out.numel() * 4 < 1e9 else ""}
             del d_series
+
+    # channel shards: the band sum is the one place where ranks exchange data -- every rank sums its own channels on the
+    # common time axis (the shard's shifts are the whole band's rows), one all-reduce of n_dm x n_series floats follows
+    band_ar = None
+    if by_channels and world > 1:
+        n_ser = plan.band_samples(n_out)
+        if n_ser > 0:
+            part = plan.band_sum(d_out)
+            torch.cuda.synchronize()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            dist.barrier()
+            a0.record()
+            dist.all_reduce(part)
+            a1.record()
+            torch.cuda.synchronize()
+            band_ar = {"collective": "nccl all_reduce(sum)", "floats": int(part.numel()),
+                       "ms": max_over_ranks(a0.elapsed_time(a1))}
 
     # ---- roofline of the dominant (fused) kernel --------------------------------------------------------------------
     peaks, peaks_src = measured_peaks()
@@ -497,10 +545,10 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "ms_per_step_stats": step_stats, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32",
+        "ms_per_step": ms_step, "ms_per_step_stats": step_stats, "higher_is_better": True,
+        "scaling": "strong" if by_channels else "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "real_time_factor": value * 1e6 / w.bw_hz,
+        "real_time_factor": value * 1e6 / w_band.bw_hz,
         "config": {"workload": w.name, "n_chan": w.n_chan, "bw_hz": w.bw_hz, "f_center_hz": w.f_center_hz,
                    "n_fft": w.n_fft, "n_int": w.n_int, "dm": list(w.dm_trials), "duration_s": w.duration_s,
                    "samples_per_channel": T, "head": head, "tail": tail, "L": L, "blocks_per_channel": nb,
@@ -508,9 +556,12 @@ def run_ours(args):
                    "output_bytes": int(d_out.numel() * 4),
                    "l2": "inputs larger than L2 (no flush needed)" if d_in.numel() > 256e6 else
                          "input smaller than 2x L2: numbers include L2 hits",
-                   "sharding": "one workload-sized batch per rank, no data-path collective"},
+                   "sharding": ("one contiguous channel range of ONE workload per rank (dedisp_plan_shard, the whole band's "
+                                "framing), no data-path collective in the step; n_chan/bw_hz/f_center_hz above are rank "
+                                "0's range") if by_channels else
+                               "one workload-sized batch per rank, no data-path collective"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps,
-        "roofline": roofline, "cpu_baseline": cpu, "cufft_reference_point": cufft_ref, "next_rows": {"band_sum": band},
+        "roofline": roofline, "cpu_baseline": cpu, "cufft_reference_point": cufft_ref, "next_rows": {"band_sum": band, "band_sum_allreduce": band_ar},
         "checksum_mean_first_1000": checksum,
     }
     print(json.dumps(line), flush=True)

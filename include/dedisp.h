@@ -84,6 +84,30 @@ int dedisp_framing(int n_chan, double bw_hz, double f_center_hz, const double* d
 int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, double f_center_hz, const double* dm, int n_dm,
                 int n_fft, int n_int, unsigned flags);
 
+/*
+ * A plan for channels chan0 .. chan0 + n_chan - 1 of a band of n_chan_total channels (bw_hz_total, f_center_hz_total):
+ * the unit of the two ways the path is partitioned over channels.  Every (channel, block) is independent, so there is
+ * no exchange between shards.
+ *   (a) channel-range shards on several GPUs (the paper splits the two polarisations over two hosts the
+ *       same way): shard_flags = 0.  The shard uses the framing of the WHOLE band, so all shards share
+ *       head/tail/L and one time axis; its chirp factors and band-alignment shifts are bit-identical to the matching
+ *       rows of dedisp_plan() on the whole band.  Input: the shard's own columns, int8 [n_samp][n_chan][2].
+ *   (b) per-channel-group framing on one GPU (the length to discard is the
+ *       dispersion time in the band, which falls as f^-3 across a wide band): DEDISP_SHARD_OWN_FRAMING computes
+ *       head/tail/L from the group's own sub-band (R18), so high-frequency groups keep more of every transform.  The
+ *       group's outputs start dedisp_shard_time_offset() = (head_whole - head_group)/n_int output samples EARLIER than
+ *       the whole band's: out_whole_axis[j] = out_group[j + offset].  dedisp_band_shifts() already contains the offset.
+ *   DEDISP_SHARD_FULL_INPUT: d_in of dedisp_execute() is the whole band, int8 [n_samp][n_chan_total][2], and the plan
+ *       reads its own columns (groups on one GPU); dedisp_stream_* is not available for such plans (EINVAL).
+ * Output layout and all other calls are those of a plan with n_chan channels.  Errors as dedisp_plan, plus EINVAL for a
+ * channel range outside the band.
+ */
+enum { DEDISP_SHARD_FULL_INPUT = 1u, DEDISP_SHARD_OWN_FRAMING = 2u };
+int dedisp_plan_shard(dedisp_plan_t* out_plan, int n_chan_total, double bw_hz_total, double f_center_hz_total,
+                      const double* dm, int n_dm, int n_fft, int n_int, unsigned flags, int chan0, int n_chan,
+                      unsigned shard_flags);
+long long dedisp_shard_time_offset(dedisp_plan_t plan); /* 0 for dedisp_plan() and for shards with the band's framing */
+
 int dedisp_get_info(dedisp_plan_t plan, dedisp_info_t* info);
 
 /* Outputs per (dm, channel) of a one-shot call on n_samp samples per channel: nb*L/n_int with

@@ -14,7 +14,7 @@ TAPER = {"none": 0, "hann": 1, "welch": 2}
 
 # every symbol include/dedisp.h declares (tests check that the library exports all of them)
 SYMBOLS = (
-    "dedisp_framing", "dedisp_plan", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
+    "dedisp_framing", "dedisp_plan", "dedisp_plan_shard", "dedisp_shard_time_offset", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
     "dedisp_execute_add",
     "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_profile_enable",
     "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_fold", "dedisp_destroy",
@@ -46,6 +46,10 @@ def _load() -> C.CDLL:
     dp, ip, vp, ll = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p, C.c_longlong
     L.dedisp_framing.argtypes = [C.c_int, C.c_double, C.c_double, dp, C.c_int, C.c_int, C.c_int, ip, ip, ip]
     L.dedisp_plan.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, dp, C.c_int, C.c_int, C.c_int, C.c_uint]
+    L.dedisp_plan_shard.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, dp, C.c_int, C.c_int, C.c_int, C.c_uint,
+                                    C.c_int, C.c_int, C.c_uint]
+    L.dedisp_shard_time_offset.argtypes = [vp]
+    L.dedisp_shard_time_offset.restype = ll
     L.dedisp_get_info.argtypes = [vp, C.POINTER(Info)]
     L.dedisp_out_samples.argtypes = [vp, ll]
     L.dedisp_out_samples.restype = ll
@@ -105,6 +109,17 @@ def dedisp_plan(n_chan: int, bw_hz: float, f_center_hz: float, dm: Sequence[floa
     return Plan(n_chan, bw_hz, f_center_hz, dm, n_fft, n_int, taper)
 
 
+SHARD_FULL_INPUT, SHARD_OWN_FRAMING = 1, 2
+
+
+def dedisp_plan_shard(n_chan_total: int, bw_hz_total: float, f_center_hz_total: float, dm: Sequence[float], n_fft: int,
+                      n_int: int, chan0: int, n_chan: int, taper: str = "none", full_input: bool = False,
+                      own_framing: bool = False) -> "Plan":
+    """Plan for channels chan0 .. chan0 + n_chan - 1 of the band (dedisp.h: dedisp_plan_shard)."""
+    return Plan(n_chan_total, bw_hz_total, f_center_hz_total, dm, n_fft, n_int, taper,
+                shard=(chan0, n_chan, (SHARD_FULL_INPUT if full_input else 0) | (SHARD_OWN_FRAMING if own_framing else 0)))
+
+
 UBENCH_FORMS = ("plain 2xFADD2", "times-i 2xFADD2 (lane-swapped operand)", "twiddle conventional FMUL2+FFMA2+2xFADD2",
                 "twiddle folded 3xFFMA2 (v=2a-u)", "twiddle folded, rotated by i", "twiddle folded 4xFFMA2",
                 "immediate twiddle folded 3xFFMA2", "immediate twiddle conventional")
@@ -132,11 +147,19 @@ def dedisp_fold(d_series, t0_s: float, dt_s: float, period_s: float, n_bins: int
 class Plan:
     """Owns a dedisp_plan_t.  Methods take torch tensors (or raw pointers) and pass pointers through."""
 
-    def __init__(self, n_chan, bw_hz, f_center_hz, dm, n_fft, n_int, taper="none"):
+    def __init__(self, n_chan, bw_hz, f_center_hz, dm, n_fft, n_int, taper="none", shard=None):
         self._h = C.c_void_p()
         arr, n = _dm_array(dm)
-        _check(_lib.dedisp_plan(C.byref(self._h), n_chan, bw_hz, f_center_hz, arr, n, n_fft, n_int, TAPER[taper]),
-               "dedisp_plan")
+        if shard is None:
+            _check(_lib.dedisp_plan(C.byref(self._h), n_chan, bw_hz, f_center_hz, arr, n, n_fft, n_int, TAPER[taper]),
+                   "dedisp_plan")
+            self.in_chan = n_chan
+        else:
+            chan0, n_shard, sflags = shard
+            _check(_lib.dedisp_plan_shard(C.byref(self._h), n_chan, bw_hz, f_center_hz, arr, n, n_fft, n_int,
+                                          TAPER[taper], chan0, n_shard, sflags), "dedisp_plan_shard")
+            self.in_chan = n_chan if sflags & SHARD_FULL_INPUT else n_shard  # channels per row of execute()'s input
+        self.time_offset = int(_lib.dedisp_shard_time_offset(self._h))
         info = Info()
         _check(_lib.dedisp_get_info(self._h, C.byref(info)), "dedisp_get_info")
         self.info = info
@@ -159,7 +182,7 @@ class Plan:
         add=True: dedisp_execute_add, the intensities are added to d_out (second polarisation)."""
         import torch
         assert d_in.is_cuda and d_in.dtype == torch.int8 and d_in.is_contiguous()
-        assert d_in.dim() == 3 and d_in.shape[1] == self.n_chan and d_in.shape[2] == 2
+        assert d_in.dim() == 3 and d_in.shape[1] == self.in_chan and d_in.shape[2] == 2
         assert not add or d_out is not None, "add=True needs the first polarisation's output"
         n_samp = d_in.shape[0]
         n_out = self.out_samples(n_samp)

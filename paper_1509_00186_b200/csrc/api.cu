@@ -40,19 +40,32 @@ static void free_plan(dedisp_plan_s* p)
     delete p;
 }
 
-extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, double f_center_hz, const double* dm,
-                           int n_dm, int n_fft, int n_int, unsigned flags)
+// dedisp_plan and dedisp_plan_shard: channels chan0 .. chan0 + n_chan - 1 of a band of n_chan_total channels.
+static int plan_impl(dedisp_plan_t* out_plan, int n_chan_total, double bw_total, double F_total, const double* dm, int n_dm,
+                     int n_fft, int n_int, unsigned flags, int chan0, int n_chan, unsigned shard_flags)
 {
     if (!out_plan) return DEDISP_EINVAL;
     *out_plan = nullptr;
     if ((flags & ~DEDISP_TAPER_MASK) || (flags & DEDISP_TAPER_MASK) == 3u) return DEDISP_EINVAL;
+    if (shard_flags & ~(DEDISP_SHARD_FULL_INPUT | DEDISP_SHARD_OWN_FRAMING)) return DEDISP_EINVAL;
     if (n_fft <= 0 || (n_fft & (n_fft - 1)) || !dedisp_aos_supported(n_fft)) return DEDISP_EINVAL;
     // R9 gives D_tot % n_int == 0, so L % n_int == n_fft % n_int: only powers of two can divide a block evenly
     if (n_int <= 0 || (n_int & (n_int - 1))) return DEDISP_EINVAL;
-    int head, tail, L;
+    if (n_chan_total <= 0 || chan0 < 0 || n_chan <= 0 || chan0 > n_chan_total - n_chan) return DEDISP_EINVAL;
+    // the whole band's framing: the common time axis of all shards (R9), and the one a plain plan uses
+    int head_w, tail_w, L_w;
     double smear = 0.0;
-    int rc = dedisp_framing_impl(n_chan, bw_hz, f_center_hz, dm, n_dm, n_fft, n_int, &head, &tail, &L, &smear);
+    int rc = dedisp_framing_impl(n_chan_total, bw_total, F_total, dm, n_dm, n_fft, n_int, &head_w, &tail_w, &L_w, &smear);
     if (rc != DEDISP_OK) return rc;
+    const double dv_total = bw_total / n_chan_total;
+    const double bw_hz = dv_total * n_chan;                                               // this plan's sub-band
+    const double f_center_hz = F_total - 0.5 * bw_total + ((double)chan0 + 0.5 * n_chan) * dv_total;
+    int head = head_w, tail = tail_w, L = L_w;
+    if (shard_flags & DEDISP_SHARD_OWN_FRAMING) {  // per-channel-group framing: only this group's own smear (R18)
+        rc = dedisp_framing_impl(n_chan, bw_hz, f_center_hz, dm, n_dm, n_fft, n_int, &head, &tail, &L, &smear);
+        if (rc != DEDISP_OK) return rc;
+        if (head > head_w) return DEDISP_EINVAL;  // cannot happen: a sub-band's delays are bounded by the band's
+    }
 
     int dev = 0, n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) {
@@ -69,6 +82,9 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     memset(p, 0, sizeof(*p));
     p->n_chan = n_chan; p->n_dm = n_dm; p->n_fft = n_fft; p->n_int = n_int;
     p->bw_hz = bw_hz; p->f_center_hz = f_center_hz; p->flags = flags;
+    p->n_chan_total = n_chan_total; p->chan0 = chan0; p->bw_total_hz = bw_total; p->f_center_total_hz = F_total;
+    p->in_pitch = (shard_flags & DEDISP_SHARD_FULL_INPUT) ? n_chan_total : n_chan;
+    p->time_offset = (head_w - head) / n_int;  // both are multiples of n_int (R9)
     p->head = head; p->tail = tail; p->L = L; p->device = dev;
     p->max_smear_samples = smear;
     {   // P:L139-141 length rule, advisory
@@ -80,24 +96,26 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     if (!p->dm) { free_plan(p); return DEDISP_ENOMEM; }
     memcpy(p->dm, dm, sizeof(double) * n_dm);
 
-    {   // band alignment (R16): delay of channel c against the top channel in whole output samples, minimum removed
+    {   // band alignment (R16): delay of channel c against the top channel of the WHOLE band in whole output samples,
+        // the whole band's minimum removed, plus this plan's time offset against the whole band's framing: the
+        // shifted outputs of all shards of one band line up sample for sample
         p->band_shift = (long long*)malloc(sizeof(long long) * (size_t)n_dm * n_chan);
         if (!p->band_shift) { free_plan(p); return DEDISP_ENOMEM; }
-        const double dv = bw_hz / n_chan, f_top = f_center_hz + 0.5 * bw_hz - 0.5 * dv;
+        const double f_top = F_total + 0.5 * bw_total - 0.5 * dv_total;
         p->band_max_shift = 0;
         for (int d = 0; d < n_dm; ++d) {
             long long* sh = p->band_shift + (size_t)d * n_chan;
-            long long lo = 0;
-            for (int c = 0; c < n_chan; ++c) {
-                const double fc = f_center_hz - 0.5 * bw_hz + ((double)c + 0.5) * dv;
+            long long lo = 0, hi = 0;
+            for (int c = 0; c < n_chan_total; ++c) {
+                const double fc = F_total - 0.5 * bw_total + ((double)c + 0.5) * dv_total;
                 const double delay_s = DEDISP_D_HZ2_S * dm[d] * (1.0 / (fc * fc) - 1.0 / (f_top * f_top));
-                sh[c] = llround(delay_s * dv / (double)n_int);
-                if (c == 0 || sh[c] < lo) lo = sh[c];
+                const long long v = llround(delay_s * dv_total / (double)n_int);
+                if (c == 0 || v < lo) lo = v;
+                if (c == 0 || v > hi) hi = v;
+                if (c >= chan0 && c < chan0 + n_chan) sh[c - chan0] = v;
             }
-            for (int c = 0; c < n_chan; ++c) {
-                sh[c] -= lo;
-                if (sh[c] > p->band_max_shift) p->band_max_shift = sh[c];
-            }
+            for (int c = 0; c < n_chan; ++c) sh[c] += p->time_offset - lo;
+            if (hi - lo + p->time_offset > p->band_max_shift) p->band_max_shift = hi - lo + p->time_offset;
         }
     }
     double* d_dm = nullptr;
@@ -139,6 +157,22 @@ extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, do
     return DEDISP_OK;
 }
 
+extern "C" int dedisp_plan(dedisp_plan_t* out_plan, int n_chan, double bw_hz, double f_center_hz, const double* dm,
+                           int n_dm, int n_fft, int n_int, unsigned flags)
+{
+    return plan_impl(out_plan, n_chan, bw_hz, f_center_hz, dm, n_dm, n_fft, n_int, flags, 0, n_chan, 0u);
+}
+
+extern "C" int dedisp_plan_shard(dedisp_plan_t* out_plan, int n_chan_total, double bw_hz_total, double f_center_hz_total,
+                                 const double* dm, int n_dm, int n_fft, int n_int, unsigned flags, int chan0, int n_chan,
+                                 unsigned shard_flags)
+{
+    return plan_impl(out_plan, n_chan_total, bw_hz_total, f_center_hz_total, dm, n_dm, n_fft, n_int, flags, chan0, n_chan,
+                     shard_flags);
+}
+
+extern "C" long long dedisp_shard_time_offset(dedisp_plan_t p) { return p ? p->time_offset : 0; }
+
 extern "C" int dedisp_get_info(dedisp_plan_t p, dedisp_info_t* info)
 {
     if (!p || !info) return DEDISP_EINVAL;
@@ -167,7 +201,8 @@ int dedisp_enqueue_chunk(dedisp_plan_s* p, const int8_t* d_in, long long n_rows,
     cudaEvent_t* ev = nullptr;
     if (p->prof_on && p->prof_n < DEDISP_PROF_MAX) ev = p->prof_ev + 3 * (p->prof_n++);
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[0], st));
-    int rc = dedisp_launch_corner_turn(d_in, n_rows, p->n_chan, d_xt, xt_stride, dst_t0, st);
+    int rc = dedisp_launch_corner_turn(d_in, n_rows, p->n_chan, p->in_pitch, p->in_pitch == p->n_chan ? 0 : p->chan0, d_xt,
+                                       xt_stride, dst_t0, st);
     if (rc != DEDISP_OK) return rc;
     if (ev) DEDISP_CUDA_TRY(cudaEventRecord(ev[1], st));
     if (after_corner_turn) DEDISP_CUDA_TRY(cudaEventRecord(after_corner_turn, st));
@@ -320,7 +355,8 @@ static int debug_prepare(dedisp_plan_t p, const int8_t* d_in, long long n_samp, 
     if (block < 0 || block >= nb) return DEDISP_EINVAL;
     int rc = dedisp_reserve(p, n_samp);
     if (rc != DEDISP_OK) return rc;
-    return dedisp_launch_corner_turn(d_in, nb * p->L + p->head + p->tail, p->n_chan, p->d_xt, p->xt_cap_samp, 0, st);
+    return dedisp_launch_corner_turn(d_in, nb * p->L + p->head + p->tail, p->n_chan, p->in_pitch,
+                                     p->in_pitch == p->n_chan ? 0 : p->chan0, p->d_xt, p->xt_cap_samp, 0, st);
 }
 
 extern "C" int dedisp_debug_unpack(dedisp_plan_t p, const int8_t* d_in, long long n_samp, int chan, long long block,

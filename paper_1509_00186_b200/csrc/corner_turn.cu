@@ -17,8 +17,8 @@ constexpr int PITCH_W = 33;  // smem row pitch in 32-bit words (64 shorts + 1 wo
 // 8-sample grid (the first tile starts dst_t0 % 8 rows before row 0), so any dst_t0 keeps the 16 B stores aligned:
 // the streaming path appends chunks behind a carry of arbitrary length.
 __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const int8_t* __restrict__ in, long long n_samp, int n_chan,
-                                                              int8_t* __restrict__ xt, long long xt_stride,
-                                                              long long dst_t0)
+                                                              int in_pitch, int8_t* __restrict__ xt,
+                                                              long long xt_stride, long long dst_t0)
 {
     __shared__ uint32_t tile[TILE_T * PITCH_W];
     const long long t0 = (long long)blockIdx.x * TILE_T - (dst_t0 & 7);
@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const int8_t* __re
         const int c = c0 + q * 8;
         uint4 v = make_uint4(0, 0, 0, 0);
         if (t >= 0 && t < n_samp && c < n_chan)  // n_chan % 8 == 0: the 8 channels are all inside
-            v = __ldg(reinterpret_cast<const uint4*>(in16 + t * n_chan + c));
+            v = __ldg(reinterpret_cast<const uint4*>(in16 + t * in_pitch + c));
         v.x ^= 0x80808080u; v.y ^= 0x80808080u; v.z ^= 0x80808080u; v.w ^= 0x80808080u;
         uint32_t* dst = &tile[row * PITCH_W + q * 4];
         dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const int8_t* __re
 
 // Scalar path for any n_chan / alignment: 32 x 32 tile of 2-byte samples.
 __global__ void __launch_bounds__(256) corner_turn_scalar_kernel(const int8_t* __restrict__ in, long long n_samp,
-                                                                 int n_chan, int8_t* __restrict__ xt,
+                                                                 int n_chan, int in_pitch, int8_t* __restrict__ xt,
                                                                  long long xt_stride, long long dst_t0)
 {
     __shared__ uint16_t tile[32][33];
@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(256) corner_turn_scalar_kernel(const int8_t* _
     for (int r = y; r < 32; r += 8) {
         const long long t = t0 + r;
         const int c = c0 + x;
-        tile[r][x] = (t < n_samp && c < n_chan) ? (uint16_t)(in16[t * n_chan + c] ^ 0x8080u) : (uint16_t)0x8080u;
+        tile[r][x] = (t < n_samp && c < n_chan) ? (uint16_t)(in16[t * in_pitch + c] ^ 0x8080u) : (uint16_t)0x8080u;
     }
     __syncthreads();
     for (int r = y; r < 32; r += 8) {
@@ -93,18 +93,19 @@ __global__ void __launch_bounds__(256) corner_turn_scalar_kernel(const int8_t* _
 
 }  // namespace
 
-int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int8_t* d_xt, long long xt_stride,
-                              long long dst_t0, cudaStream_t st)
+int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int in_pitch, int chan0, int8_t* d_xt,
+                              long long xt_stride, long long dst_t0, cudaStream_t st)
 {
     if (n_samp <= 0) return DEDISP_OK;
-    const bool vec = (n_chan % 8 == 0) && (xt_stride % 8 == 0) && ((uintptr_t)d_in % 16 == 0) &&
+    d_in += 2 * (size_t)chan0;  // first column of this plan's channels
+    const bool vec = (n_chan % 8 == 0) && (in_pitch % 8 == 0) && (xt_stride % 8 == 0) && ((uintptr_t)d_in % 16 == 0) &&
                      ((uintptr_t)d_xt % 16 == 0);
     if (vec) {
         dim3 grid((unsigned)((n_samp + (dst_t0 & 7) + TILE_T - 1) / TILE_T), (unsigned)((n_chan + TILE_C - 1) / TILE_C));
-        corner_turn_vec_kernel<<<grid, 256, 0, st>>>(d_in, n_samp, n_chan, d_xt, xt_stride, dst_t0);
+        corner_turn_vec_kernel<<<grid, 256, 0, st>>>(d_in, n_samp, n_chan, in_pitch, d_xt, xt_stride, dst_t0);
     } else {
         dim3 grid((unsigned)((n_samp + 31) / 32), (unsigned)((n_chan + 31) / 32));
-        corner_turn_scalar_kernel<<<grid, 256, 0, st>>>(d_in, n_samp, n_chan, d_xt, xt_stride, dst_t0);
+        corner_turn_scalar_kernel<<<grid, 256, 0, st>>>(d_in, n_samp, n_chan, in_pitch, d_xt, xt_stride, dst_t0);
     }
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;

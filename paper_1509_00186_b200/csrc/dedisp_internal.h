@@ -14,7 +14,13 @@ struct dedisp_stream_state;
 struct dedisp_plan_s {
     // problem statement (observing frequency, bandwidth, DM) + channelisation and transform sizes
     int n_chan, n_dm, n_fft, n_int;
-    double bw_hz, f_center_hz;
+    double bw_hz, f_center_hz;  // of THIS plan's channels (a shard: its sub-band)
+    // the whole band this plan's channels are cut from (dedisp_plan_shard; equal to the above for dedisp_plan): the
+    // chirp and the band-alignment shifts are computed from these, so a shard's values are bit-identical to the whole plan's
+    int n_chan_total, chan0;
+    double bw_total_hz, f_center_total_hz;
+    int in_pitch;               // channels per row of the caller's input: n_chan, or n_chan_total (DEDISP_SHARD_FULL_INPUT)
+    long long time_offset;      // output samples by which this plan's time axis is ahead of the whole band's framing
     double* dm;  // host copy [n_dm]
     unsigned flags;
     // framing (R9)
@@ -58,8 +64,9 @@ static inline long long dedisp_xt_stride(long long n_samp) { return (n_samp + 63
 
 // corner_turn.cu (all launchers enqueue only)
 // corner turn: int8 [n_samp][n_chan][2] -> int8 [n_chan][xt_stride][2], rows t0_dst.. of the destination
-int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int8_t* d_xt, long long xt_stride,
-                              long long dst_t0, cudaStream_t st);
+// (columns chan0 .. chan0 + n_chan - 1 of rows that are in_pitch channels wide)
+int dedisp_launch_corner_turn(const int8_t* d_in, long long n_samp, int n_chan, int in_pitch, int chan0, int8_t* d_xt,
+                              long long xt_stride, long long dst_t0, cudaStream_t st);
 // fused_aos.cu: fused unpack -> forward FFT -> chirp -> inverse FFT -> discard -> detect -> integrate over nb blocks of
 // every channel (all enqueue only):  out[d][c][out_col0 + b*L/n_int + j]
 // accumulate != 0: add to d_out instead of overwriting it

@@ -76,14 +76,15 @@ extern "C" int dedisp_framing(int n_chan, double bw_hz, double f_center_hz, cons
 // ---------------------------------------------------------------------------------------------------------------
 // chirp[d][c][k] = w(f_k) * exp(-2 pi i psi) / N,  psi = D DM f^2 / ((f + f_c) f_c^2) cycles: the inverse of
 // the ISM's in-band term, which Eq. 3 prints as exp(+2 pi i psi); R1, R2
+// (bw, F, n_chan_total describe the WHOLE band; the table holds channels chan0 .. chan0 + n_chan - 1 of it)
 __global__ void chirp_table_kernel(float2* __restrict__ chirp, const double* __restrict__ dm, int n_chan, int n_fft,
-                                   double bw, double F, unsigned taper)
+                                   double bw, double F, int n_chan_total, int chan0, unsigned taper)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int c = blockIdx.y, d = blockIdx.z;
     if (k >= n_fft) return;
-    const double dv = bw / (double)n_chan;
-    const double fc = chan_center_hz(F, bw, n_chan, c);
+    const double dv = bw / (double)n_chan_total;
+    const double fc = chan_center_hz(F, bw, n_chan_total, chan0 + c);
     const int ks = (k < n_fft / 2) ? k : k - n_fft;  // bin N/2 is -dv/2 (R5)
     const double f = (double)ks * dv / (double)n_fft;
     double psi = DEDISP_D_HZ2_S * dm[d] * f * f / ((f + fc) * fc * fc);
@@ -113,8 +114,8 @@ __global__ void twiddle_table_kernel(float2* __restrict__ tw, int n_fft)
 int dedisp_launch_chirp_table(const dedisp_plan_s* p, const double* d_dm, cudaStream_t st)
 {
     dim3 grid((p->n_fft + 255) / 256, p->n_chan, p->n_dm);
-    chirp_table_kernel<<<grid, 256, 0, st>>>(p->d_chirp, d_dm, p->n_chan, p->n_fft, p->bw_hz, p->f_center_hz,
-                                             p->flags & DEDISP_TAPER_MASK);
+    chirp_table_kernel<<<grid, 256, 0, st>>>(p->d_chirp, d_dm, p->n_chan, p->n_fft, p->bw_total_hz, p->f_center_total_hz,
+                                             p->n_chan_total, p->chan0, p->flags & DEDISP_TAPER_MASK);
     DEDISP_CUDA_TRY(cudaGetLastError());
     return DEDISP_OK;
 }

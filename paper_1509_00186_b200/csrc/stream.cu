@@ -54,6 +54,7 @@ void dedisp_stream_free(dedisp_plan_s* p)
 extern "C" int dedisp_stream_begin(dedisp_plan_t p, long long max_chunk_samp)
 {
     if (!p || max_chunk_samp <= 0) return DEDISP_EINVAL;
+    if (p->in_pitch != p->n_chan) return DEDISP_EINVAL;  // DEDISP_SHARD_FULL_INPUT plans: one-shot calls only
     if (p->stream && p->stream->max_chunk >= max_chunk_samp) {
         // a new observation on buffers that are already big enough: drain, forget the carry, keep the allocations
         int rc = dedisp_stream_sync(p);

@@ -711,3 +711,40 @@ def test_p20_unpack_block_is_the_framed_slice_of_the_input():
             assert got.dtype == np.float64 and got.shape == (cfg.n_fft, 2)
             assert np.array_equal(got, x[b * L: b * L + cfg.n_fft, c, :].astype(np.float64))
     assert (x == -128).any()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P21 (R18): per-channel-group framing.  A group of channels framed for its OWN smear (P:L121,
+# the length to discard is the dispersion time in the band; it falls as f^-3) gives the same
+# dedispersed series as the whole-band framing, shifted by the whole number (head_whole - head_group)/n_int of outputs
+# ----------------------------------------------------------------------------------------------------------------
+def test_p21_group_framing_retimes_to_the_whole_band_axis():
+    n_int = 4
+    whole = oracle.OracleConfig(8, 16e6, 60e6, (0.001,), 1024, n_int)       # 52 ... 68 MHz: smear falls 2.2x across it
+    head_w, tail_w, L_w = oracle.framing(whole)
+    x = datagen.noise_only(12 * 1024, 8, seed=31)
+    ref = oracle.dedisp(whole, x)
+    # an impulse in every channel at one instant: the position is fixed by the sample grid, not by a correlation
+    xi = np.zeros((6 * 1024, 8, 2), dtype=np.int8)
+    t_imp = 2500
+    xi[t_imp, :, 0] = 100
+    ref_i = oracle.dedisp(whole, xi)
+    heads = []
+    for g in range(2):
+        c0, n = 4 * g, 4
+        cfg = oracle.OracleConfig(n, n * 2e6, 60e6 - 8e6 + (c0 + 0.5 * n) * 2e6, (0.001,), 1024, n_int)
+        head, tail, L = oracle.framing(cfg)
+        heads.append(head)
+        assert head <= head_w and tail <= tail_w and L >= L_w and (head_w - head) % n_int == 0
+        off = (head_w - head) // n_int
+        out = oracle.dedisp(cfg, np.ascontiguousarray(x[:, c0:c0 + n]))
+        m = min(ref.shape[2], out.shape[2] - off)
+        a, b = ref[:, c0:c0 + n, :m], out[:, :, off:off + m]
+        rel = np.sqrt(((a - b) ** 2).sum() / (a ** 2).sum())
+        rel_off = np.sqrt(((a[:, :, 1:] - b[:, :, :-1]) ** 2).sum() / (a ** 2).sum())
+        assert rel < 0.02 < 0.2 < rel_off, (g, rel, rel_off)   # aligned: wrap-around differences only (see P5)
+        # the dedispersed energy of the impulse peaks in the same output sample on the common axis, for every channel
+        out_i = oracle.dedisp(cfg, np.ascontiguousarray(xi[:, c0:c0 + n]))
+        for c in range(n):
+            assert int(np.argmax(out_i[0, c])) - off == int(np.argmax(ref_i[0, c0 + c]))
+    assert heads[1] < heads[0] == head_w                         # the low group sets the band's framing
