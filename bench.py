@@ -74,6 +74,9 @@ def parse_args():
     ap.add_argument("--shard", choices=("batches", "channels"), default="batches",
                     help="N > 1: one workload-sized batch per rank (weak scaling, default) or one channel range of ONE "
                          "workload per rank (strong scaling, dedisp_plan_shard; SURVEY 8(e), P:L256-258)")
+    ap.add_argument("--groups", type=int, default=0,
+                    help="G > 1: time the workload as G channel groups, each framed for its own smear "
+                         "(dedisp_plan_shard + DEDISP_SHARD_OWN_FRAMING, SURVEY 8(f) NEXT-2), beside the one-framing plan")
     ap.add_argument("--duration", type=float, default=0.0, help="override the workload's seconds of data (debug)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -570,6 +573,56 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_groups(args):
+    """--groups G: per-channel-group framing (NEXT-2, DESIGN R18) against the one-framing plan on the same input, one GPU.
+    Both produce the same dedispersed series on the common time axis (tests/test_gpu_shards.py); what changes is how
+    many VALID samples every transform yields, so the comparison is time per step for the same data."""
+    import torch
+    import datagen
+    import paper_1509_00186_b200 as dd
+    torch.cuda.set_device(0)
+    w = get_workload(args, 0)
+    d_in = torch.from_numpy(datagen.generate(w)).cuda()
+    T, G = d_in.shape[0], args.groups
+
+    def timed(plans):
+        outs = [torch.empty((p.n_dm, p.n_chan, p.out_samples(T)), dtype=torch.float32, device="cuda") for p in plans]
+        for p in plans:
+            p.reserve(T)
+        for _ in range(max(args.warmup, 3)):
+            for p, o in zip(plans, outs):
+                p.execute(d_in, o)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            for p, o in zip(plans, outs):
+                p.execute(d_in, o)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    one = dd.dedisp_plan(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int)
+    ms_one = timed([one])
+    groups = []
+    for g in range(G):
+        c0, n = channel_shard(w.n_chan, g, G)
+        groups.append(dd.dedisp_plan_shard(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int, c0, n,
+                                           full_input=True, own_framing=True))
+    ms_grp = timed(groups)
+    # the data both cover: the common output range on the whole band's time axis, in input samples per channel
+    common = min([one.out_samples(T)] + [p.out_samples(T) - p.time_offset for p in groups]) * w.n_int
+    line = {"metric": METRIC, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "config": {"workload": w.name, "groups": G, "n_fft": w.n_fft, "n_dm": len(w.dm_trials)},
+            "one_framing": {"ms_per_step": ms_one, "L": one.L, "value": w.n_chan * common / (ms_one * 1e-3) / 1e6},
+            "group_framing": {"ms_per_step": ms_grp, "L": [p.L for p in groups],
+                              "L_mean": sum(p.L * p.n_chan for p in groups) / w.n_chan,
+                              "time_offset": [p.time_offset for p in groups],
+                              "value": w.n_chan * common / (ms_grp * 1e-3) / 1e6},
+            "speedup": ms_one / ms_grp, "higher_is_better": True, "data": "synthetic", "dtype": "f32"}
+    print(json.dumps(line), flush=True)
+
+
 def run_ubench(args):
     """--ubench fp32-issue: SM sub-partition cycles per radix-2 butterfly for every instruction form of
     dedisp_ubench_fp32 (csrc/ubench.cu); the numbers DESIGN.md section 6 quotes come from this command."""
@@ -589,7 +642,9 @@ def run_ubench(args):
 
 def main():
     args = parse_args()
-    if args.ubench:
+    if args.groups > 1:
+        run_groups(args)
+    elif args.ubench:
         run_ubench(args)
     elif args.impl == "reference":
         run_reference(args)
