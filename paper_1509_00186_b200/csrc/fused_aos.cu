@@ -26,6 +26,7 @@
 // forward transform places before its first scatter); the chirp row is rewritten between two __syncthreads() that all
 // units reach in the same loop iteration.
 #include <mutex>
+#include <type_traits>
 
 #include "dedisp_internal.h"
 #include "fft_aos.cuh"
@@ -253,22 +254,46 @@ __global__ void __launch_bounds__((Cfg<N, E>::CTA), 1) fused_aos_kernel(const Ao
                 const bool writer = live && (t & ((1 << LPO) - 1)) == 0;
                 if (PIPE && s + s_step < s_end) unpack(s + s_step);  // beside the shared-memory reads below
                 const int n_full = n_work / TPU, rem = n_work - n_full * TPU;
-                auto one = [&](int i, bool valid) {
-                    float acc = 0.f;
-                    if (valid) {
-                        const float4 u = p4[i * TPU];
-                        acc = (u.x + u.y) + (u.z + u.w);
-                    }
+                constexpr int QS = TPU >> LPO;  // stride of a thread's outputs
+                // four chunks per trip: the loads go out together with immediate offsets, the pointers move once, the
+                // stores are predicated on one loop-invariant flag; no reconvergence point inside the loop
+                auto run = [&](auto acc_tag) {
+                    constexpr bool ACC = decltype(acc_tag)::value;
+                    const float4* pp = p4;
+                    float* q = dt;
+                    auto sum4 = [](const float4& u) { return (u.x + u.y) + (u.z + u.w); };
+                    auto reduce = [](float v) {
 #pragma unroll
-                    for (int off = 1; off < (1 << LPO); off <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-                    if (writer && valid) {
-                        float* q = dt + i * (TPU >> LPO);
-                        *q = a.accumulate ? *q + acc : acc;
+                        for (int off = 1; off < (1 << LPO); off <<= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+                        return v;
+                    };
+                    int i = 0;
+#pragma unroll 1
+                    for (; i + 4 <= n_full; i += 4) {
+                        const float4 u0 = pp[0], u1 = pp[TPU], u2 = pp[2 * TPU], u3 = pp[3 * TPU];
+                        const float r0 = reduce(sum4(u0)), r1 = reduce(sum4(u1)), r2 = reduce(sum4(u2)),
+                                    r3 = reduce(sum4(u3));
+                        if (writer) {
+                            if (ACC) { q[0] += r0; q[QS] += r1; q[2 * QS] += r2; q[3 * QS] += r3; }
+                            else { q[0] = r0; q[QS] = r1; q[2 * QS] = r2; q[3 * QS] = r3; }
+                        }
+                        pp += 4 * TPU;
+                        q += 4 * QS;
+                    }
+#pragma unroll 1
+                    for (; i < n_full + (rem > 0 ? 1 : 0); ++i) {  // the last trip may be ragged: rem % 2^LPO == 0
+                        const bool valid = i < n_full || t < rem;
+                        const float r = reduce(valid ? sum4(pp[0]) : 0.f);
+                        if (writer && valid) {
+                            if (ACC) q[0] += r;
+                            else q[0] = r;
+                        }
+                        pp += TPU;
+                        q += QS;
                     }
                 };
-#pragma unroll 4
-                for (int i = 0; i < n_full; ++i) one(i, true);
-                if (rem > 0) one(n_full, t < rem);
+                if (a.accumulate) run(std::true_type{});
+                else run(std::false_type{});
             } else {
                 for (int id = t; id - t < n_work; id += TPU) {  // uniform trip count: the shuffles need whole warps
                     float acc = 0.f;
