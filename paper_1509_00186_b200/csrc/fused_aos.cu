@@ -83,13 +83,20 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // biased int8 pair ((re ^ 0x80) | (im ^ 0x80) << 8, as the corner turn stores it: u = x + 128) -> fp32 (re, im), exact,
 // without I2F: PRMT builds 0x4B0000uu = 2^23 + u, then one packed add of -(2^23 + 128)
-__device__ __forceinline__ C unpack_int8x2(uint32_t w)
+__device__ __forceinline__ C unpack_int8x2(uint32_t w, uint32_t k /* 0x4B000000 */)
 {
-    const uint32_t k = 0x4B000000u;
     uint32_t re, im;
     asm("prmt.b32 %0, %1, %2, 0x7440;" : "=r"(re) : "r"(w), "r"(k));
     asm("prmt.b32 %0, %1, %2, 0x7441;" : "=r"(im) : "r"(w), "r"(k));
     return __fadd2_rn(make_float2(__uint_as_float(re), __uint_as_float(im)), make_float2(-8388736.0f, -8388736.0f));
+}
+// The PRMT constant, made opaque to the compiler: left to itself it re-creates 0x4B000000 with an HFMA2 (an FP32-pipe
+// instruction) before every conversion instead of keeping it in one register.
+__device__ __forceinline__ uint32_t magic_2p23()
+{
+    uint32_t k;
+    asm volatile("mov.b32 %0, 0x4B000000;" : "=r"(k));
+    return k;
 }
 
 template <int N, int E> constexpr size_t smem_bytes()
@@ -164,17 +171,19 @@ __global__ void __launch_bounds__((Cfg<N, E>::CTA), 1) fused_aos_kernel(const Ao
 
     // 1b. unpack int8 (re, im) -> fp32 (exact) for this thread's unit of super-item s2
     C x[E];
+    const uint32_t k23 = magic_2p23();
     auto unpack = [&](int s2) {
-        const int c2 = s2 / a.spc;
-        const int b2 = (s2 - c2 * a.spc) * UPS + us;
-        const bool live2 = b2 < a.nb;
+        // (a unit slot past the channel's last block is transformed like the others -- any bytes are valid samples --
+        // and only its stores are suppressed: no select per element here)
         if constexpr (STAGE) {
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = unpack_int8x2(live2 ? (uint32_t)stage[t + m * TPU] : 0u);
+            for (int m = 0; m < E; ++m) x[m] = unpack_int8x2((uint32_t)stage[t + m * TPU], k23);
         } else {  // block b reads rows b*L .. b*L+N-1 (P:L270 framing)
+            const int c2 = s2 / a.spc;
+            const int b2 = min((s2 - c2 * a.spc) * UPS + us, a.nb - 1);
             const uint16_t* src = xt16 + (long long)c2 * a.xt_stride + (long long)b2 * a.L + t;
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = unpack_int8x2(live2 ? (uint32_t)__ldg(src + m * TPU) : 0u);
+            for (int m = 0; m < E; ++m) x[m] = unpack_int8x2((uint32_t)__ldg(src + m * TPU), k23);
         }
     };
     // PIPE (single-DM plans): the unpack of the NEXT super-item runs beside the epilogue of this one, whose
