@@ -186,10 +186,11 @@ __device__ __forceinline__ void pass_dit(C (&x)[E], const TwBase<E, R>& tb)
     for (int q = 0; q < E / R; ++q) dft_dit<E, R, SIGN, TW>(x, q, tb.w[q]);
 }
 
-// Exchange buffer: one 8-byte cell of padding per P cells, P = the first pass's radix, keeps the strided STS.64 of the
-// first exchange (thread t writes cells t*P .. t*P + P - 1) and every contiguous access free of bank conflicts (a
-// 64-bit access is served 16 lanes at a time: (P + 1) t mod 16 = t).
-template <int P> __host__ __device__ constexpr int padp(int i) { return i + i / P; }
+// Exchange buffer: two 8-byte cells of padding per P cells, P = the first pass's radix.  In the first exchange thread t
+// writes cells t*P .. t*P + P - 1, two at a time with STS.128: rows of P + 2 cells start 16-byte aligned, and a quarter
+// warp's eight stores (served together) fall (P + 2) * 8 bytes = 16 (mod 128) apart: no bank conflict.  Every other access
+// is contiguous across threads (64-bit, served 16 lanes at a time).
+template <int P> __host__ __device__ constexpr int padp(int i) { return i + 2 * (i / P); }
 
 // Exchange through shared memory, in two halves so that the caller can place its barrier (and work that only needs the
 // barrier, like a prefetch) between them: scatter the pass outputs to their Stockham positions; [barrier]; gather the
@@ -202,14 +203,21 @@ __device__ __forceinline__ void exchange_scatter(const C (&x)[E], int t, C* __re
     static_assert(NS == 1 ? R == P : NS % P == 0, "padp(j0 + r*NS) must split into padp(j0) + constant");
     // NS == 1: output r of butterfly j goes to cell j*R + r, j*R a multiple of P = R; otherwise r*NS is a multiple of
     // P: either way the padded position of output r is padp(j0) plus a compile-time constant (base + immediate).
-    constexpr int STEP = NS == 1 ? 1 : NS + NS / P;
+    constexpr int STEP = NS == 1 ? 1 : NS + 2 * (NS / P);
 #pragma unroll
     for (int q = 0; q < S; ++q) {
         const int jv = t + q * TPU;
         const int k = jv & (NS - 1);
         C* base = sm + padp<P>((jv - k) * R + k);
+        if constexpr (NS == 1) {  // adjacent cells: 16-byte stores
 #pragma unroll
-        for (int r = 0; r < R; ++r) base[r * STEP] = x[q + r * S];
+            for (int r = 0; r < R; r += 2)
+                *reinterpret_cast<float4*>(base + r) =
+                    make_float4(x[q + r * S].x, x[q + r * S].y, x[q + (r + 1) * S].x, x[q + (r + 1) * S].y);
+        } else {
+#pragma unroll
+            for (int r = 0; r < R; ++r) base[r * STEP] = x[q + r * S];
+        }
     }
 }
 
