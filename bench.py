@@ -15,7 +15,12 @@ e2e        the same metric through dedisp_stream_push() on pinned HOST buffers i
 roofline   the fused kernel (dominant): nominal flops of its launches / its CUDA-event time (the library's
            dedisp_profile_* events on the launching stream) against the FP32 FMA peak (bound "alu").
 cpu_baseline   the fp64 oracle, as it stands, on the host cores, on a bounded leading slice of the same input.
-N > 1      every rank runs its own workload-sized batch (its own seed): no data-path collective, "scaling": "weak".
+N > 1      every rank runs its own workload-sized batch (its own seed): no data-path collective, "scaling": "weak";
+           --shard channels: every rank one channel range of ONE workload (dedisp_plan_shard), "scaling": "strong".
+other_workloads   (default run only) step and fused-kernel time of the other four BASELINE.json configs, device-resident,
+           so that every roofline fraction DESIGN.md quotes is measured by the driver's own run (wideband on a 1 s cut).
+--groups G        per-channel-group framing against the one-framing plan (its own JSON line).
+--ubench fp32-issue   cycle cost of the butterfly forms (its own JSON line).
 """
 from __future__ import annotations
 
@@ -81,6 +86,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT+elementwise reference point")
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the short device-resident runs of the other four BASELINE.json workloads (other_workloads)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the cpu_baseline leg")
     ap.add_argument("--ubench", choices=("fp32-issue",), default=None,
                     help="run a micro-benchmark instead of the bench (one JSON line; not the bench contract)")
@@ -546,6 +553,14 @@ def run_ours(args):
                "sample": f"first {nb_cpu} of {nb_all} blocks of every channel ({dt:.1f} s of wall time)",
                "real_time_factor": rate * 1e6 / w.bw_hz}
 
+    others = None
+    if world == 1 and not args.no_others and args.workload == "gmrt32" and not by_channels and args.duration == 0:
+        try:
+            del h_in
+            others = measure_other_workloads(max(3, min(args.steps, 10)), fp32_peak_tf)
+        except Exception as exc:            # an extra: it must never take the headline down
+            others = {"error": repr(exc)[:200]}
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "ms_per_step_stats": step_stats, "higher_is_better": True,
@@ -564,13 +579,61 @@ def run_ours(args):
                                 "0's range") if by_channels else
                                "one workload-sized batch per rank, no data-path collective"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps,
-        "roofline": roofline, "cpu_baseline": cpu, "cufft_reference_point": cufft_ref, "next_rows": {"band_sum": band, "band_sum_allreduce": band_ar},
+        "roofline": roofline, "cpu_baseline": cpu, "cufft_reference_point": cufft_ref, "next_rows": {"band_sum": band, "band_sum_allreduce": band_ar}, "other_workloads": others,
         "checksum_mean_first_1000": checksum,
     }
     print(json.dumps(line), flush=True)
     plan.destroy()
     if world > 1:
         dist.destroy_process_group()
+
+
+OTHER_WORKLOADS = (("tiny", 0.0), ("gmrt16", 0.0), ("lowfreq", 0.0), ("wideband", 1.0))   # (name, seconds; 0 = full)
+
+
+def measure_other_workloads(steps: int, fp32_peak_tf: float):
+    """Device-resident step and fused-kernel time of the other four BASELINE.json configs, so that their roofline
+    fractions are measured by the same run as the headline (wideband on a 1 s cut of its 8 s: 2048 channels x 15
+    blocks x 8 DMs, 207 units per SM).  Same method as the headline: CUDA events around `steps` dedisp_execute
+    calls, the library's own events around the fused kernel."""
+    import torch
+    import datagen
+    import paper_1509_00186_b200 as dd
+    out = {}
+    for name, dur in OTHER_WORKLOADS:
+        w = datagen.WORKLOADS[name]
+        if dur > 0:
+            w = w.scaled(dur)
+        d_in = torch.from_numpy(datagen.generate(w)).cuda()
+        T = d_in.shape[0]
+        with dd.dedisp_plan(w.n_chan, w.bw_hz, w.f_center_hz, w.dm_trials, w.n_fft, w.n_int) as plan:
+            nb, n_out = plan.n_blocks(T), plan.out_samples(T)
+            plan.reserve(T)
+            d_out = torch.empty((plan.n_dm, w.n_chan, n_out), dtype=torch.float32, device="cuda")
+            for _ in range(3):
+                plan.execute(d_in, d_out)
+            torch.cuda.synchronize()
+            plan.profile_enable(True)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                plan.execute(d_in, d_out)
+            e1.record()
+            torch.cuda.synchronize()
+            ms_ct, ms_fused, n_prof = plan.profile_read()
+            plan.profile_enable(False)
+            ms_step = e0.elapsed_time(e1) / steps
+            fused_ms = ms_fused / max(n_prof, 1)
+            units = w.n_chan * nb
+            tf = units * nominal_flops_per_unit(w.n_fft, plan.L, plan.n_dm) / (fused_ms * 1e-3) / 1e12
+            out[name] = {"duration_s": w.duration_s, "n_fft": w.n_fft, "n_dm": plan.n_dm, "n_int": w.n_int,
+                         "units": units, "ms_per_step": ms_step, "value": units * plan.L / (ms_step * 1e-3) / 1e6,
+                         "real_time_factor": units * plan.L / (ms_step * 1e-3) / w.bw_hz,
+                         "fused_ms_per_launch": fused_ms, "fused_frac_of_fp32_peak": tf / fp32_peak_tf,
+                         "corner_turn_ms_per_launch": ms_ct / max(n_prof, 1)}
+        del d_in, d_out
+        torch.cuda.empty_cache()
+    return out
 
 
 def run_groups(args):
