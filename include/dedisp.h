@@ -226,6 +226,35 @@ int dedisp_debug_chirp(dedisp_plan_t plan, int d, int chan, float* h_chirp);
 int dedisp_debug_voltage(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, int chan, long long block,
                          float* d_volt, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Full-band mode: the paper's own pipeline, no sub-banding (Fig. 4; SURVEY 8(f)
+ * NEXT-1; readings R19-R21; oracle: oracle/fullband.py).
+ *   1. every GSB spectrum (int8 [n_chan][2]: bins 0 .. n_chan-1 of a 2 n_chan-point real FFT, R19) is inverse
+ *      transformed to 2 n_chan real samples: the Nyquist-sampled voltage series v
+ *   2. blocks of n_fft samples (block b reads v[b L : b L + n_fft]) go through ONE long transform
+ *   3. bin k (f_l = k 2 bw / n_fft above the lower band edge f_lo, R21) is multiplied by
+ *      w(f_l) exp(-2 pi i psi), psi = D DM f_l^2 / ((f_l + f_lo) f_lo^2): Eq. 3 inverted, taper P:L123
+ *   4. inverse transform; 5. the first D outputs of a block are dropped (R20; D = dispersion time in samples at
+ *      2 bw, rounded up to n_int), L = n_fft - D stay; 6. squared and summed in groups of n_int
+ *   out[d][b L/n_int + j] = sum_{i < n_int} y_d[b][D + j n_int + i]^2
+ *   n_chan: 512 ... 8192 (2 n_chan a power of two); n_fft: a power of two in 2^20 ... 2^28; dm >= 0 (HOST, copied).
+ * dedisp_fullband_framing is pure host arithmetic.  execute: DEVICE pointers, enqueues on the stream, allocates its
+ * scratch on first use.  Errors as above (ESHORT: fewer than n_fft samples).
+ * ------------------------------------------------------------------------------------------------------------------ */
+typedef struct dedisp_fullband_s* dedisp_fullband_t;
+int dedisp_fullband_framing(double bw_hz, double f_lo_hz, const double* dm, int n_dm, long long n_fft, int n_int, int* D,
+                            long long* L);
+int dedisp_fullband_plan(dedisp_fullband_t* out_plan, int n_chan, double bw_hz, double f_lo_hz, const double* dm, int n_dm,
+                         long long n_fft, int n_int, unsigned flags);
+int dedisp_fullband_get_framing(dedisp_fullband_t plan, int* D, long long* L, int* n1, int* n2); /* n_fft = n1 * n2 */
+long long dedisp_fullband_out_samples(dedisp_fullband_t plan, long long n_spec);
+int dedisp_fullband_execute(dedisp_fullband_t plan, const int8_t* d_spec, long long n_spec, float* d_out,
+                            long long out_stride, void* cuda_stream); /* d_spec [n_spec][n_chan][2], d_out [n_dm][out_stride] */
+/* test hook: step 1 alone, float [n_spec * 2 n_chan] on the DEVICE */
+int dedisp_fullband_debug_series(dedisp_fullband_t plan, const int8_t* d_spec, long long n_spec, float* d_series,
+                                 void* cuda_stream);
+int dedisp_fullband_destroy(dedisp_fullband_t plan);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,6 +20,8 @@ SYMBOLS = (
     "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_fold", "dedisp_destroy",
     "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
     "dedisp_ubench_fp32",
+    "dedisp_fullband_framing", "dedisp_fullband_plan", "dedisp_fullband_get_framing", "dedisp_fullband_out_samples",
+    "dedisp_fullband_execute", "dedisp_fullband_debug_series", "dedisp_fullband_destroy",
 )
 
 
@@ -50,6 +52,15 @@ def _load() -> C.CDLL:
                                     C.c_int, C.c_int, C.c_uint]
     L.dedisp_shard_time_offset.argtypes = [vp]
     L.dedisp_shard_time_offset.restype = ll
+    llp = C.POINTER(ll)
+    L.dedisp_fullband_framing.argtypes = [C.c_double, C.c_double, dp, C.c_int, ll, C.c_int, ip, llp]
+    L.dedisp_fullband_plan.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, dp, C.c_int, ll, C.c_int, C.c_uint]
+    L.dedisp_fullband_get_framing.argtypes = [vp, ip, llp, ip, ip]
+    L.dedisp_fullband_out_samples.argtypes = [vp, ll]
+    L.dedisp_fullband_out_samples.restype = ll
+    L.dedisp_fullband_execute.argtypes = [vp, vp, ll, vp, ll, vp]
+    L.dedisp_fullband_debug_series.argtypes = [vp, vp, ll, vp, vp]
+    L.dedisp_fullband_destroy.argtypes = [vp]
     L.dedisp_get_info.argtypes = [vp, C.POINTER(Info)]
     L.dedisp_out_samples.argtypes = [vp, ll]
     L.dedisp_out_samples.restype = ll
@@ -301,3 +312,69 @@ class Plan:
 
     def __exit__(self, *exc):
         self.destroy()
+
+
+def dedisp_fullband_framing(bw_hz: float, f_lo_hz: float, dm: Sequence[float], n_fft: int, n_int: int):
+    """(D, L) of the full-band mode (dedisp.h: dedisp_fullband_framing); host arithmetic only."""
+    arr, n = _dm_array(dm)
+    d, l = C.c_int(), C.c_longlong()
+    _check(_lib.dedisp_fullband_framing(bw_hz, f_lo_hz, arr, n, n_fft, n_int, C.byref(d), C.byref(l)),
+           "dedisp_fullband_framing")
+    return d.value, l.value
+
+
+class FullbandPlan:
+    """Owns a dedisp_fullband_t: the paper's own full-band mode (dedisp.h).  Argument marshalling only."""
+
+    def __init__(self, n_chan, bw_hz, f_lo_hz, dm, n_fft, n_int, taper="none"):
+        self._h = C.c_void_p()
+        arr, n = _dm_array(dm)
+        _check(_lib.dedisp_fullband_plan(C.byref(self._h), n_chan, bw_hz, f_lo_hz, arr, n, n_fft, n_int, TAPER[taper]),
+               "dedisp_fullband_plan")
+        d, l, n1, n2 = C.c_int(), C.c_longlong(), C.c_int(), C.c_int()
+        _check(_lib.dedisp_fullband_get_framing(self._h, C.byref(d), C.byref(l), C.byref(n1), C.byref(n2)),
+               "dedisp_fullband_get_framing")
+        self.n_chan, self.n_dm, self.n_fft, self.n_int = n_chan, n, n_fft, n_int
+        self.D, self.L, self.n1, self.n2 = d.value, l.value, n1.value, n2.value
+
+    def out_samples(self, n_spec: int) -> int:
+        return int(_lib.dedisp_fullband_out_samples(self._h, n_spec))
+
+    def execute(self, d_spec, d_out=None, stream=None):
+        """d_spec: CUDA int8 [n_spec][n_chan][2] -> CUDA float32 [n_dm][n_out]."""
+        import torch
+        assert d_spec.is_cuda and d_spec.dtype == torch.int8 and d_spec.is_contiguous()
+        assert d_spec.dim() == 3 and d_spec.shape[1] == self.n_chan and d_spec.shape[2] == 2
+        n_out = self.out_samples(d_spec.shape[0])
+        if d_out is None:
+            d_out = torch.empty((self.n_dm, max(n_out, 0)), dtype=torch.float32, device=d_spec.device)
+        assert d_out.is_cuda and d_out.dtype == torch.float32 and d_out.is_contiguous() and d_out.shape[0] == self.n_dm
+        st = torch.cuda.current_stream(d_spec.device).cuda_stream if stream is None else stream
+        _check(_lib.dedisp_fullband_execute(self._h, d_spec.data_ptr(), d_spec.shape[0], d_out.data_ptr(),
+                                            d_out.shape[1], st), "dedisp_fullband_execute")
+        return d_out
+
+    def debug_series(self, d_spec):
+        import torch
+        out = torch.empty(d_spec.shape[0] * 2 * self.n_chan, dtype=torch.float32, device=d_spec.device)
+        st = torch.cuda.current_stream(d_spec.device).cuda_stream
+        _check(_lib.dedisp_fullband_debug_series(self._h, d_spec.data_ptr(), d_spec.shape[0], out.data_ptr(), st),
+               "dedisp_fullband_debug_series")
+        return out
+
+    def destroy(self):
+        if self._h:
+            _lib.dedisp_fullband_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
