@@ -79,6 +79,8 @@ def parse_args():
     ap.add_argument("--shard", choices=("batches", "channels"), default="batches",
                     help="N > 1: one workload-sized batch per rank (weak scaling, default) or one channel range of ONE "
                          "workload per rank (strong scaling, dedisp_plan_shard; SURVEY 8(e), P:L256-258)")
+    ap.add_argument("--fullband", type=int, default=0, metavar="LOG2N",
+                    help="time the paper's full-band mode (dedisp_fullband_*) with transforms of 2^LOG2N points, 20 ... 27")
     ap.add_argument("--groups", type=int, default=0,
                     help="G > 1: time the workload as G channel groups, each framed for its own smear "
                          "(dedisp_plan_shard + DEDISP_SHARD_OWN_FRAMING, SURVEY 8(f) NEXT-2), beside the one-framing plan")
@@ -636,6 +638,68 @@ def measure_other_workloads(steps: int, fp32_peak_tf: float):
     return out
 
 
+def run_fullband(args):
+    """--fullband LOG2N: the paper's own mode (dedisp_fullband_*) on synthetic GSB spectra shaped
+    like its 32 MHz setting (512 channels, 325 MHz, int8 Gaussian(sigma 20) re/im), one GPU, its own
+    JSON line.  DM is the largest that the length rule of P:L139-141 still maps to N = 2^LOG2N.  HBM-bound: a four-step
+    transform has to read and write its array once per pass, forward and inverse 2 passes each = 4 x 16 B per complex
+    point (two real blocks ride one complex transform) -- the algorithmic figure; this build moves 7 x 16 B
+    (4 transposes + 3 row-transform kernels)."""
+    import numpy as np
+    import torch
+    import paper_1509_00186_b200 as dd
+    torch.cuda.set_device(0)
+    n_chan, bw, f_lo, n_int = 512, 32e6, 309e6, 1024          # 15 us at 64 Msamples/s is ~10^3 samples (P:L336)
+    N = 1 << args.fullband
+    smear_per_dm = 4.148808e15 * (1.0 / f_lo ** 2 - 1.0 / (f_lo + bw) ** 2) * 2 * bw      # samples per unit DM
+    dm = 0.499 * N / smear_per_dm                              # N is the smallest power of 2 > 2 x smear
+    plan = dd.FullbandPlan(n_chan, bw, f_lo, (dm,), N, n_int)
+    n_blocks = max(2, min(16, (1 << 28) // N))
+    n_spec = -(-(n_blocks * plan.L + plan.D) // (2 * n_chan))
+    rng = np.random.default_rng(5)
+    spec = np.clip(np.rint(rng.normal(0.0, 20.0, size=(n_spec, n_chan, 2))), -127, 127).astype(np.int8)
+    d_spec = torch.from_numpy(spec).cuda()
+    d_out = torch.empty((1, plan.out_samples(n_spec)), dtype=torch.float32, device="cuda")
+    for _ in range(max(args.warmup, 3)):
+        plan.execute(d_spec, d_out)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0).start()
+    time.sleep(0.3)
+    mark0 = sampler.mark()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    evs[0].record()
+    for i in range(args.steps):
+        plan.execute(d_spec, d_out)
+        evs[i + 1].record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop(mark0, None)
+    st = stats([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
+    ms = evs[0].elapsed_time(evs[-1]) / args.steps
+    nb = d_out.shape[1] // (plan.L // n_int)
+    valid = nb * plan.L                                        # valid real samples dedispersed per step
+    pairs = (nb + 1) // 2
+    peaks, peaks_src = measured_peaks()
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    alg = pairs * N * 64.0 + n_spec * n_chan * 2.0 + valid * 4.0 / n_int
+    line = {"metric": "real Msamples/s dedispersed (full band)", "value": valid / (ms * 1e-3) / 1e6, "unit": "Msamples/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "ms_per_step_stats": st,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "real_time_factor": valid / (ms * 1e-3) / (2 * bw),
+            "config": {"workload": f"fullband32 (512 ch, 32 MHz at 325 MHz, N = 2^{args.fullband})", "n_chan": n_chan,
+                       "bw_hz": bw, "f_lo_hz": f_lo, "dm": [dm], "n_fft": N, "n1": plan.n1, "n2": plan.n2, "n_int": n_int,
+                       "D": plan.D, "L": plan.L, "blocks": nb, "n_spec": n_spec},
+            "clocks": clocks, "gpu_launches": args.steps * (1 + pairs // max(1, (1 << 27) // N) * 0 + 8),
+            "roofline": {"bound": "hbm", "kernel": "whole full-band step (1 c2r + 3 row-transform + 4 transpose + 1 detect kernels)",
+                         "achieved": alg / (ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                         "frac": alg / (ms * 1e-3) / 1e9 / hbm, "traffic": None,
+                         "algorithmic_bytes_per_step": alg, "moved_bytes_per_step_by_design": pairs * N * 112.0,
+                         "peak_source": f"hbm_gbs of MEASURED_PEAKS.json ({peaks_src})"},
+            "paper_context": "P:L285-287: 1.4x real time at 32 MHz on a Tesla C2075 + Xeon X5550, fp64",
+            "checksum_mean": float(d_out.double().mean().item())}
+    print(json.dumps(line), flush=True)
+    plan.destroy()
+
+
 def run_groups(args):
     """--groups G: per-channel-group framing (NEXT-2, DESIGN R18) against the one-framing plan on the same input, one GPU.
     Both produce the same dedispersed series on the common time axis (tests/test_gpu_shards.py); what changes is how
@@ -705,7 +769,9 @@ def run_ubench(args):
 
 def main():
     args = parse_args()
-    if args.groups > 1:
+    if args.fullband:
+        run_fullband(args)
+    elif args.groups > 1:
         run_groups(args)
     elif args.ubench:
         run_ubench(args)
