@@ -28,7 +28,10 @@ using namespace dedisp_aos;
 
 namespace {
 
-constexpr int FB_E = 64, FB_CTA = 256;
+constexpr int FB_E = 64;
+// threads per CTA of the row kernels: two units where a unit is small enough -- two such CTAs share an SM and drift apart,
+// so that one's loads and stores overlap the other's butterflies -- else one unit
+template <int R> __host__ __device__ constexpr int fb_cta() { return R / FB_E >= 128 ? R / FB_E : 128; }
 template <int N> struct FShape;
 template <> struct FShape<1024>  { static constexpr int R0 = 64, R1 = 16, R2 = 1, R3 = 1; };
 template <> struct FShape<2048>  { static constexpr int R0 = 64, R1 = 32, R2 = 1, R3 = 1; };
@@ -66,10 +69,10 @@ struct RowsArgs {
 //   ROWS_TWIDDLE_INV  out[row] = IDFT( in[row][k] * conj(W_N^{(row in transform) * k}) )       (steps 2'-1')
 //   ROWS_GSB          series[row*R + n] = Re IDFT(Hermitian extension of gsb[row])[n] / R      (R19: c2r of a spectrum)
 template <int R, int MODE>
-__global__ void __launch_bounds__(FB_CTA, 1) fb_rows_kernel(const RowsArgs a)
+__global__ void __launch_bounds__((fb_cta<R>()), (fb_cta<R>() == 128 ? 2 : 1)) fb_rows_kernel(const RowsArgs a)
 {
     using Sh = FShape<R>;
-    constexpr int E = FB_E, TPU = R / E, UPS = FB_CTA / TPU, P = Sh::R0, GROUP = TPU < 32 ? 32 : TPU;
+    constexpr int E = FB_E, TPU = R / E, FB_CTA = fb_cta<R>(), UPS = FB_CTA / TPU, P = Sh::R0, GROUP = TPU < 32 ? 32 : TPU;
     extern __shared__ float2 smem2[];
     const int us = threadIdx.x / TPU, t = threadIdx.x % TPU;
     const int bar_id = threadIdx.x / GROUP + 1;
@@ -81,12 +84,13 @@ __global__ void __launch_bounds__(FB_CTA, 1) fb_rows_kernel(const RowsArgs a)
     C x[E];
     if constexpr (MODE == ROWS_GSB) {
         // bins 0 .. R/2-1 are recorded (bin 0: real part only), bin R/2 is 0, the rest is the conjugate mirror (R19)
-        const int8_t* g = a.gsb + r * R;  // (R/2 bins x 2 bytes)
+        const uint16_t* g = reinterpret_cast<const uint16_t*>(a.gsb) + r * (R / 2);  // one (re, im) byte pair per bin
 #pragma unroll
         for (int m = 0; m < E; ++m) {
             const int k = t + m * TPU;
             const int ks = k < R / 2 ? k : R - k;
-            const float re = (float)g[2 * (ks & (R / 2 - 1))], im = (float)g[2 * (ks & (R / 2 - 1)) + 1];
+            const uint32_t w = __ldg(g + (ks & (R / 2 - 1)));
+            const float re = (float)(int8_t)(w & 0xffu), im = (float)(int8_t)(w >> 8);
             x[m] = k == R / 2 ? make_float2(0.f, 0.f)
                               : (k == 0 ? make_float2(re, 0.f) : make_float2(re, k < R / 2 ? im : -im));
         }
@@ -239,7 +243,7 @@ __global__ void fb_chirp_kernel(float2* __restrict__ chirp, int n1, int n2, doub
     chirp[idx] = make_float2((float)(w * c), (float)((k <= n / 2 ? -1.0 : 1.0) * w * s));
 }
 
-template <int R> constexpr size_t rows_smem() { return (size_t)(FB_CTA / (R / FB_E)) * padp<FShape<R>::R0>(R) * sizeof(float2); }
+template <int R> constexpr size_t rows_smem() { return (size_t)(fb_cta<R>() / (R / FB_E)) * padp<FShape<R>::R0>(R) * sizeof(float2); }
 
 template <int R, int MODE> int launch_rows_r(const RowsArgs& a, cudaStream_t st)
 {
@@ -251,7 +255,7 @@ template <int R, int MODE> int launch_rows_r(const RowsArgs& a, cudaStream_t st)
                                              (int)rows_smem<R>()));
         attr_set[dev] = true;
     }
-    constexpr int UPS = FB_CTA / (R / FB_E);
+    constexpr int FB_CTA = fb_cta<R>(), UPS = FB_CTA / (R / FB_E);
     const long long grid = (a.n_rows + UPS - 1) / UPS;
     if (grid <= 0 || grid > 0x7fffffffll) return DEDISP_EINVAL;
     fb_rows_kernel<R, MODE><<<(unsigned)grid, FB_CTA, rows_smem<R>(), st>>>(a);
