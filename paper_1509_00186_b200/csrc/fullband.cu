@@ -160,6 +160,52 @@ __global__ void __launch_bounds__(256) fb_transpose_kernel(const float2* __restr
     for (int j = ty; j < 32; j += 8) out[batch * mat + (size_t)(c0 + j) * rows + r0 + tx] = tile[tx][j];
 }
 
+// The last transpose of the inverse transform fused with the detection (n_int a multiple of 32): a tile row of the
+// transposed result is 32 consecutive samples n of one block pair, all inside one integration group, so instead of
+// writing y the warp squares and adds them: part[batch][0/1][n / 32] = sum of re^2 (block 2 batch) / im^2 (the block
+// after it).  Saves the 8 B per point store and fb_detect_kernel's 8 B per point read; fb_sum_parts_kernel adds
+// n_int/32 consecutive partial sums per output in a fixed order (no atomics: results are reproducible).
+__global__ void __launch_bounds__(256) fb_transpose_detect_kernel(const float2* __restrict__ in, float* __restrict__ part,
+                                                                  int rows, int cols)
+{
+    __shared__ float2 tile[32][33];
+    const size_t batch = blockIdx.z, mat = (size_t)rows * cols;
+    const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int j = ty; j < 32; j += 8) tile[j][tx] = in[batch * mat + (size_t)(r0 + j) * cols + c0 + tx];
+    __syncthreads();
+#pragma unroll
+    for (int j = ty; j < 32; j += 8) {
+        const float2 v = tile[tx][j];  // natural-order element n = (c0 + j) * rows + r0 + tx
+        float a = v.x * v.x, b = v.y * v.y;
+#pragma unroll
+        for (int off = 16; off; off >>= 1) {
+            a += __shfl_xor_sync(0xffffffffu, a, off);
+            b += __shfl_xor_sync(0xffffffffu, b, off);
+        }
+        if (tx == 0) {
+            const size_t g = ((size_t)(c0 + j) * rows + r0) >> 5;  // group of 32 samples inside the transform
+            part[(2 * batch) * (mat >> 5) + g] = a;
+            part[(2 * batch + 1) * (mat >> 5) + g] = b;
+        }
+    }
+}
+__global__ void fb_sum_parts_kernel(const float* __restrict__ part, long long groups_per_block, int D, int n_int,
+                                    long long outs_per_block, long long first_block, long long n_blocks_total,
+                                    long long n_ids, float* __restrict__ out)
+{
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= n_ids) return;
+    const long long lb = id / outs_per_block, j = id - lb * outs_per_block;  // lb = block index inside this batch set
+    const long long block = first_block + lb;
+    if (block >= n_blocks_total) return;
+    const float* p = part + lb * groups_per_block + ((long long)D + j * n_int) / 32;
+    float acc = 0.f;
+    for (int i = 0; i < n_int / 32; ++i) acc += p[i];
+    out[block * outs_per_block + j] = acc;
+}
+
 // Overlap-save discard, detect, integrate (R20): y[batch][n] complex, re = block
 // first_block + 2 batch, im = the block after it; out[block L/n_int + j] = sum_{i < n_int} part(y[D + j n_int + i])^2.
 // One warp per output when n_int >= 32, one thread otherwise.
@@ -482,11 +528,20 @@ extern "C" int dedisp_fullband_execute(dedisp_fullband_t p, const int8_t* d_spec
             // steps 2'-1': conjugate twiddle, inverse transforms of length n1
             a.in = Cc; a.out = B; a.tw = p->d_tw1; a.n_rows = (long long)pb * n2; a.rows_per_batch = n2;
             if ((rc = launch_rows<ROWS_TWIDDLE_INV>(n1, a, st)) != DEDISP_OK) return rc;
-            fb_transpose_kernel<false><<<dim3(n1 / 32, n2 / 32, pb), 256, 0, st>>>(B, Cc, n2, n1, nullptr, 0, 0, 0);  // natural order
-            // overlap-save discard, detect, integrate
-            const long long ids = (long long)pb * 2 * opb * (p->n_int >= 32 ? 32 : 1);
-            fb_detect_kernel<<<(unsigned)((ids + 255) / 256), 256, 0, st>>>(Cc, p->n_fft, p->D, p->n_int, opb, 2 * p0, nb,
-                                                                            d_out + (size_t)d * out_stride);
+            // back to natural order + overlap-save discard, detect, integrate
+            if (p->n_int % 32 == 0) {
+                float* part = reinterpret_cast<float*>(Cc);  // [pb][2][n_fft / 32]
+                fb_transpose_detect_kernel<<<dim3(n1 / 32, n2 / 32, pb), 256, 0, st>>>(B, part, n2, n1);
+                const long long ids = (long long)pb * 2 * opb;
+                fb_sum_parts_kernel<<<(unsigned)((ids + 255) / 256), 256, 0, st>>>(part, p->n_fft / 32, p->D, p->n_int, opb,
+                                                                                   2 * p0, nb, ids,
+                                                                                   d_out + (size_t)d * out_stride);
+            } else {
+                fb_transpose_kernel<false><<<dim3(n1 / 32, n2 / 32, pb), 256, 0, st>>>(B, Cc, n2, n1, nullptr, 0, 0, 0);
+                const long long ids = (long long)pb * 2 * opb * (p->n_int >= 32 ? 32 : 1);
+                fb_detect_kernel<<<(unsigned)((ids + 255) / 256), 256, 0, st>>>(Cc, p->n_fft, p->D, p->n_int, opb, 2 * p0,
+                                                                                nb, d_out + (size_t)d * out_stride);
+            }
         }
     }
     DEDISP_CUDA_TRY(cudaGetLastError());
