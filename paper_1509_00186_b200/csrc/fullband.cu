@@ -13,8 +13,9 @@
 //     2^27 points makes two passes over the data; the spectrum is left in the four-step's own order [k1][k2] -- the
 //     chirp table is stored in that order and the inverse runs the steps backwards, so no reordering pass exists.
 //   * forward rows -> chirp -> inverse rows is ONE kernel (the spectrum of a row never leaves the registers).
-//   * HBM-bound: 7 passes of 8 B read + 8 B written per complex point (4 transposes, 3 row-transform kernels), fp32
-//     values, twiddles and chirp from fp64 phases (the paper's fp64 requirement, concerns the phase: F7).
+//   * HBM-bound: 7 passes of 8 B read + 8 B written per complex point (4 transposes, 3 row-transform kernels; the last
+//     transpose writes 32-sample partial power sums instead of its result when n_int % 32 == 0), fp32 values, twiddles
+//     and chirp from fp64 phases (the paper's fp64 requirement, concerns the phase: pin F7).
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
