@@ -43,7 +43,8 @@ enum {
     DEDISP_ENOMEM = -2, /* host or device allocation failed */
     DEDISP_ECUDA = -3,  /* a CUDA call failed; dedisp_last_cuda_error() gives the cudaError_t */
     DEDISP_ESHORT = -4, /* n_samp shorter than one block (n_fft samples) */
-    DEDISP_ENODEV = -5  /* no sm_100 device / no CUDA driver */
+    DEDISP_ENODEV = -5, /* no sm_100 device / no CUDA driver */
+    DEDISP_ETOOBIG = -6 /* dedisp_execute_static: the call needs more than DEDISP_STATIC_SCRATCH_BYTES of scratch */
 };
 
 /* flags of dedisp_plan(): taper of the chirp function (P:L123 names Hanning and Welch; R6 gives the formulas) */
@@ -109,6 +110,23 @@ int dedisp_plan_shard(dedisp_plan_t* out_plan, int n_chan_total, double bw_hz_to
 long long dedisp_shard_time_offset(dedisp_plan_t plan); /* 0 for dedisp_plan() and for shards with the band's framing */
 
 int dedisp_get_info(dedisp_plan_t plan, dedisp_info_t* info);
+
+/*
+ * dedisp_execute() for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): same arguments, same kernels, same outputs, but the channel-major int8 scratch
+ * [n_chan][stride][2] that dedisp_execute() allocates on demand is a static device array of
+ * DEDISP_STATIC_SCRATCH_BYTES here (held by every GPU that loads the library until the process exits).  The call makes
+ * no cudaMalloc / cudaFree / allocating library call.
+ *   Limit: 2 * n_chan * roundup(nb*L + head + tail, 64) <= DEDISP_STATIC_SCRATCH_BYTES, else DEDISP_ETOOBIG (64 MiB holds
+ *   a 1 s chunk of the 32 MHz / 512-channel mode).  Feed longer inputs in pieces that overlap by head + tail samples.
+ *   All plans and all calls share the array and it keeps the last call's contents (nothing in it needs to start at zero: a
+ *   call reads only what its own corner turn wrote); calls that overlap on the GPU -- two streams, or two host threads
+ *   -- RACE on it: order them on one stream.  The array's device address is looked up once per device, at the first
+ *   call with that device current.
+ */
+#define DEDISP_STATIC_SCRATCH_BYTES (64u << 20)
+int dedisp_execute_static(dedisp_plan_t plan, const int8_t* d_in, long long n_samp, float* d_out, long long out_stride,
+                          void* cuda_stream);
 
 /* Outputs per (dm, channel) of a one-shot call on n_samp samples per channel: nb*L/n_int with
  * nb = floor((n_samp - head - tail)/L) (R12: no zero padding, trailing partial block dropped); 0 if too short. */

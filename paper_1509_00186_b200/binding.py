@@ -9,13 +9,13 @@ from typing import Sequence
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libdedisp.so")
 
-OK, EINVAL, ENOMEM, ECUDA, ESHORT, ENODEV = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ECUDA, ESHORT, ENODEV, ETOOBIG = 0, -1, -2, -3, -4, -5, -6
 TAPER = {"none": 0, "hann": 1, "welch": 2}
 
 # every symbol include/dedisp.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "dedisp_framing", "dedisp_plan", "dedisp_plan_shard", "dedisp_shard_time_offset", "dedisp_get_info", "dedisp_out_samples", "dedisp_reserve", "dedisp_execute",
-    "dedisp_execute_add",
+    "dedisp_execute_add", "dedisp_execute_static",
     "dedisp_stream_begin", "dedisp_stream_push", "dedisp_stream_sync", "dedisp_stream_end", "dedisp_profile_enable",
     "dedisp_profile_read", "dedisp_band_samples", "dedisp_band_shifts", "dedisp_band_sum", "dedisp_fold", "dedisp_destroy",
     "dedisp_strerror", "dedisp_last_cuda_error", "dedisp_debug_unpack", "dedisp_debug_chirp", "dedisp_debug_voltage",
@@ -67,6 +67,7 @@ def _load() -> C.CDLL:
     L.dedisp_reserve.argtypes = [vp, ll]
     L.dedisp_execute.argtypes = [vp, vp, ll, vp, ll, vp]
     L.dedisp_execute_add.argtypes = [vp, vp, ll, vp, ll, vp]
+    L.dedisp_execute_static.argtypes = [vp, vp, ll, vp, ll, vp]
     L.dedisp_stream_begin.argtypes = [vp, ll]
     L.dedisp_stream_push.argtypes = [vp, vp, ll, vp, ll, C.POINTER(ll)]
     L.dedisp_stream_sync.argtypes = [vp]
@@ -204,6 +205,19 @@ class Plan:
         st = torch.cuda.current_stream(d_in.device).cuda_stream if stream is None else stream
         fn = _lib.dedisp_execute_add if add else _lib.dedisp_execute
         _check(fn(self._h, d_in.data_ptr(), n_samp, d_out.data_ptr(), d_out.shape[2], st), "dedisp_execute")
+        return d_out
+
+    def execute_static(self, d_in, d_out, stream=None):
+        """dedisp_execute_static: execute() without any allocation (the scratch is a static 64 MiB device array shared
+        by all calls; DedispError(ETOOBIG) beyond it).  d_out must be given: this call creates nothing."""
+        import torch
+        assert d_in.is_cuda and d_in.dtype == torch.int8 and d_in.is_contiguous()
+        assert d_in.dim() == 3 and d_in.shape[1] == self.in_chan and d_in.shape[2] == 2
+        assert d_out.is_cuda and d_out.dtype == torch.float32 and d_out.is_contiguous()
+        assert d_out.dim() == 3 and d_out.shape[0] == self.n_dm and d_out.shape[1] == self.n_chan
+        st = torch.cuda.current_stream(d_in.device).cuda_stream if stream is None else stream
+        _check(_lib.dedisp_execute_static(self._h, d_in.data_ptr(), d_in.shape[0], d_out.data_ptr(), d_out.shape[2], st),
+               "dedisp_execute_static")
         return d_out
 
     def execute_ptr(self, in_ptr: int, n_samp: int, out_ptr: int, out_stride: int, stream: int = 0) -> None:

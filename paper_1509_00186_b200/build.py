@@ -12,7 +12,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libdedisp.so")
-SOURCES = ("plan.cu", "api.cu", "corner_turn.cu", "fused_aos.cu", "band_sum.cu", "stream.cu", "ubench.cu", "fullband.cu")
+SOURCES = ("plan.cu", "api.cu", "corner_turn.cu", "fused_aos.cu", "band_sum.cu", "stream.cu", "ubench.cu", "fullband.cu", "static_scratch.cu")
 NVCC_FLAGS = ("-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC")
 

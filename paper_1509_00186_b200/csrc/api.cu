@@ -16,6 +16,7 @@ extern "C" const char* dedisp_strerror(int code)
         case DEDISP_ECUDA: return "CUDA error (see dedisp_last_cuda_error)";
         case DEDISP_ESHORT: return "input shorter than one transform block";
         case DEDISP_ENODEV: return "no usable sm_100 CUDA device";
+        case DEDISP_ETOOBIG: return "input needs more than DEDISP_STATIC_SCRATCH_BYTES of static scratch";
         default: return "unknown dedisp status";
     }
 }
